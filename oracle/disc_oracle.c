@@ -1,0 +1,341 @@
+/*
+ * disc_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT.
+ *
+ * Plain, slow, obviously-correct CPU restatement of the DISC hot path
+ * (Zhen et al., "CT to Cone-beam CT Deformable Registration With Simultaneous
+ * Intensity Correction", arxiv 1204.6295; citations are PAPER.md:LINE).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+ * reference legs may build, load or call this file.  It shares no code, header,
+ * table or constant generator with paper_1204_6295_b200/ (the CUDA path) and
+ * neither imports the other.
+ *
+ * Conventions: volumes are float32, x fastest,
+ * idx = (z*ny + y)*nx + x; displacement is planar disp[c][z][y][x], c=0,1,2 =
+ * x,y,z, in voxel units of its level.  Arithmetic inside a step is fp64; the
+ * images m, s' and the field r are rounded to fp32 once, at the end of a step.
+ * Patch loops are naive (every voxel visits its whole patch, as the paper's own
+ * kernel does); variance is two-pass.  OpenMP over z only.
+ *
+ * Every function is pinned by tests/test_oracle_pins.py (closed forms,
+ * invariants, brute force, scipy special cases) -- no function is "parity
+ * unpinned" except registration accuracy on the paper's clinical data
+ * (PAPER.md:347-378), which is not reproducible here and not claimed.
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define IDX(x, y, z) (((size_t)(z) * ny + (y)) * nx + (x))
+
+static inline int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* ------------------------------------------------------------------------
+ * (b) warp: m(x) = I_m(x + r(x)), trilinear, sample position clamped to the
+ * volume.  PAPER.md:69 (I_m(x+v(x)) = I_s(x), pull-back), :75 "update the
+ * moving image", :171 kernel 5.  Reading A11: p = clamp(x + r, 0, n-1) per
+ * axis, i0 = min(floor(p), n-2), t = p - i0; an axis of length 1 has weight 0.
+ * ---------------------------------------------------------------------- */
+static inline void cell(double p, int n, int *i0, int *i1, double *t) {
+    if (p < 0.0) p = 0.0;
+    if (p > (double)(n - 1)) p = (double)(n - 1);
+    if (n < 2) { *i0 = 0; *i1 = 0; *t = 0.0; return; }
+    int i = (int)floor(p);
+    if (i > n - 2) i = n - 2;
+    *i0 = i; *i1 = i + 1; *t = p - (double)i;
+}
+
+static double trilinear(const float *I, int nx, int ny, int nz, double px, double py, double pz) {
+    int x0, x1, y0, y1, z0, z1; double tx, ty, tz;
+    cell(px, nx, &x0, &x1, &tx); cell(py, ny, &y0, &y1, &ty); cell(pz, nz, &z0, &z1, &tz);
+    double c00 = (1 - tx) * I[IDX(x0, y0, z0)] + tx * I[IDX(x1, y0, z0)];
+    double c10 = (1 - tx) * I[IDX(x0, y1, z0)] + tx * I[IDX(x1, y1, z0)];
+    double c01 = (1 - tx) * I[IDX(x0, y0, z1)] + tx * I[IDX(x1, y0, z1)];
+    double c11 = (1 - tx) * I[IDX(x0, y1, z1)] + tx * I[IDX(x1, y1, z1)];
+    double c0 = (1 - ty) * c00 + ty * c10;
+    double c1 = (1 - ty) * c01 + ty * c11;
+    return (1 - tz) * c0 + tz * c1;
+}
+
+void oracle_warp(const float *I, const float *disp, int nx, int ny, int nz, float *out) {
+    size_t N = (size_t)nx * ny * nz;
+#pragma omp parallel for schedule(static)
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) {
+                size_t i = IDX(x, y, z);
+                out[i] = (float)trilinear(I, nx, ny, nz, x + (double)disp[i], y + (double)disp[N + i],
+                                          z + (double)disp[2 * N + i]);
+            }
+}
+
+/* ------------------------------------------------------------------------
+ * (a1) patch moments.  PAPER.md:95 Eq. (3): E(X^p) = (1/n) sum x_i^p, p=1,2;
+ * PAPER.md:458 (A.4): STD = sqrt(E(X^2) - E(X)^2), i.e. population variance.
+ * Patch = cube of radius R centred at x, truncated to the
+ * volume (reading A4): n(x) = number of in-volume voxels.  Two-pass variance
+ * sum (x - mu)^2 / n, which equals E(X^2) - E(X)^2 in exact arithmetic.
+ * ---------------------------------------------------------------------- */
+static inline void patch_stats(const float *v, int nx, int ny, int nz, int R, int x, int y, int z,
+                               double *mean, double *var) {
+    int x0 = x - R < 0 ? 0 : x - R, x1 = x + R > nx - 1 ? nx - 1 : x + R;
+    int y0 = y - R < 0 ? 0 : y - R, y1 = y + R > ny - 1 ? ny - 1 : y + R;
+    int z0 = z - R < 0 ? 0 : z - R, z1 = z + R > nz - 1 ? nz - 1 : z + R;
+    double n = (double)(x1 - x0 + 1) * (y1 - y0 + 1) * (z1 - z0 + 1);
+    double s = 0.0;
+    for (int c = z0; c <= z1; ++c)
+        for (int b = y0; b <= y1; ++b)
+            for (int a = x0; a <= x1; ++a) s += v[IDX(a, b, c)];
+    double mu = s / n, q = 0.0;
+    for (int c = z0; c <= z1; ++c)
+        for (int b = y0; b <= y1; ++b)
+            for (int a = x0; a <= x1; ++a) { double d = v[IDX(a, b, c)] - mu; q += d * d; }
+    *mean = mu; *var = q / n;
+}
+
+void oracle_box_moments(const float *v, int nx, int ny, int nz, int R, double *mean, double *var) {
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) patch_stats(v, nx, ny, nz, R, x, y, z, &mean[IDX(x, y, z)], &var[IDX(x, y, z)]);
+}
+
+/* moments at a list of voxel indices only (sampled checks at sizes where the full loop takes minutes) */
+void oracle_box_moments_at(const float *v, int nx, int ny, int nz, int R, const long long *idx, int nidx,
+                           double *mean, double *var) {
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int k = 0; k < nidx; ++k) {
+        long long i = idx[k];
+        int x = (int)(i % nx), y = (int)((i / nx) % ny), z = (int)(i / ((long long)nx * ny));
+        patch_stats(v, nx, ny, nz, R, x, y, z, &mean[k], &var[k]);
+    }
+}
+
+/* ------------------------------------------------------------------------
+ * (a2) correction.  PAPER.md:117-119 Eqs. (5)-(6): a = STD(M)/STD(S),
+ * b = E(M) - a E(S); I'_s = a I_s + b applied to the ORIGINAL
+ * static image.  Written as I' = a (I_s - mu_s) + mu_m (north_star formula,
+ * identical algebra).  Reading A5: a = 0 where var_s <= eps_var.
+ * ---------------------------------------------------------------------- */
+static inline double correct_one(double Is, double mu_s, double var_s, double mu_m, double var_m, double eps_var) {
+    double a = var_s > eps_var ? sqrt(var_m / var_s) : 0.0;
+    return a * (Is - mu_s) + mu_m;
+}
+
+void oracle_correct_from_moments(const float *cbct, const double *mu_s, const double *var_s, const double *mu_m,
+                                 const double *var_m, size_t N, double eps_var, float *out) {
+#pragma omp parallel for schedule(static)
+    for (long long i = 0; i < (long long)N; ++i)
+        out[i] = (float)correct_one(cbct[i], mu_s[i], var_s[i], mu_m[i], var_m[i], eps_var);
+}
+
+void oracle_correct(const float *cbct, const float *m, int nx, int ny, int nz, int R, double eps_var, float *out) {
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) {
+                double mus, vs, mum, vm;
+                patch_stats(cbct, nx, ny, nz, R, x, y, z, &mus, &vs);
+                patch_stats(m, nx, ny, nz, R, x, y, z, &mum, &vm);
+                out[IDX(x, y, z)] = (float)correct_one(cbct[IDX(x, y, z)], mus, vs, mum, vm, eps_var);
+            }
+}
+
+void oracle_correct_at(const float *cbct, const float *m, int nx, int ny, int nz, int R, double eps_var,
+                       const long long *idx, int nidx, double *out) {
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int k = 0; k < nidx; ++k) {
+        long long i = idx[k];
+        int x = (int)(i % nx), y = (int)((i / nx) % ny), z = (int)(i / ((long long)nx * ny));
+        double mus, vs, mum, vm;
+        patch_stats(cbct, nx, ny, nz, R, x, y, z, &mus, &vs);
+        patch_stats(m, nx, ny, nz, R, x, y, z, &mum, &vm);
+        out[k] = correct_one(cbct[i], mus, vs, mum, vm, eps_var);
+    }
+}
+
+/* ------------------------------------------------------------------------
+ * (c) force + update.  PAPER.md:73 Eq. (1), first (passive) term with the
+ * corrected static image s' (Alg. A1 steps 3->4), then
+ * "add dr to the total moving vector r".  Readings A1/A7/A8:
+ * g = central difference with clamped indices, d = s' - m,
+ * r_c += d g_c / (|g|^2 + d^2 + eps_den)  (sign that descends for the
+ * pull-back warp m(x) = I_m(x + r(x))).
+ * ---------------------------------------------------------------------- */
+void oracle_force_update(const float *m, const float *s, int nx, int ny, int nz, double eps_den, float *disp) {
+    size_t N = (size_t)nx * ny * nz;
+#pragma omp parallel for schedule(static)
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) {
+                size_t i = IDX(x, y, z);
+                double gx = 0.5 * ((double)s[IDX(clampi(x + 1, 0, nx - 1), y, z)] - (double)s[IDX(clampi(x - 1, 0, nx - 1), y, z)]);
+                double gy = 0.5 * ((double)s[IDX(x, clampi(y + 1, 0, ny - 1), z)] - (double)s[IDX(x, clampi(y - 1, 0, ny - 1), z)]);
+                double gz = 0.5 * ((double)s[IDX(x, y, clampi(z + 1, 0, nz - 1))] - (double)s[IDX(x, y, clampi(z - 1, 0, nz - 1))]);
+                double d = (double)s[i] - (double)m[i];
+                double den = gx * gx + gy * gy + gz * gz + d * d + eps_den;
+                disp[i] = (float)((double)disp[i] + d * gx / den);
+                disp[N + i] = (float)((double)disp[N + i] + d * gy / den);
+                disp[2 * N + i] = (float)((double)disp[2 * N + i] + d * gz / den);
+            }
+}
+
+/* ------------------------------------------------------------------------
+ * (d) Gaussian regularisation of the total field r (Alg. A1 step 6,
+ * PAPER.md:194).  Reading A10: K = ceil(3 sigma), w_i ~ exp(-i^2 / 2 sigma^2)
+ * computed in fp64, normalised to sum 1, then rounded to fp32; replicate
+ * (clamped-index) border; passes x, y, z; direct convolution.
+ * ---------------------------------------------------------------------- */
+int oracle_gauss_radius(double sigma) { return (int)ceil(3.0 * sigma); }
+
+void oracle_gauss_weights(double sigma, float *w /* 2K+1 */) {
+    int K = oracle_gauss_radius(sigma);
+    double s = 0.0;
+    for (int i = -K; i <= K; ++i) s += exp(-(double)(i * i) / (2.0 * sigma * sigma));
+    for (int i = -K; i <= K; ++i) w[i + K] = (float)(exp(-(double)(i * i) / (2.0 * sigma * sigma)) / s);
+}
+
+static void conv_axis(const double *in, double *out, int nx, int ny, int nz, int axis, const float *w, int K) {
+#pragma omp parallel for schedule(static)
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) {
+                double acc = 0.0;
+                for (int k = -K; k <= K; ++k) {
+                    int a = x, b = y, c = z;
+                    if (axis == 0) a = clampi(x + k, 0, nx - 1);
+                    else if (axis == 1) b = clampi(y + k, 0, ny - 1);
+                    else c = clampi(z + k, 0, nz - 1);
+                    acc += (double)w[k + K] * in[IDX(a, b, c)];
+                }
+                out[IDX(x, y, z)] = acc;
+            }
+}
+
+void oracle_smooth_field(float *disp, int nx, int ny, int nz, double sigma) {
+    size_t N = (size_t)nx * ny * nz;
+    int K = oracle_gauss_radius(sigma);
+    float *w = (float *)malloc(sizeof(float) * (2 * K + 1));
+    oracle_gauss_weights(sigma, w);
+    double *a = (double *)malloc(sizeof(double) * N), *b = (double *)malloc(sizeof(double) * N);
+    for (int c = 0; c < 3; ++c) {
+        float *r = disp + c * N;
+        for (size_t i = 0; i < N; ++i) a[i] = r[i];
+        conv_axis(a, b, nx, ny, nz, 0, w, K);
+        conv_axis(b, a, nx, ny, nz, 1, w, K);
+        conv_axis(a, b, nx, ny, nz, 2, w, K);
+        for (size_t i = 0; i < N; ++i) r[i] = (float)b[i];
+    }
+    free(a); free(b); free(w);
+}
+
+/* ------------------------------------------------------------------------
+ * pyramid (reading A9).  Down: 2x2x2 block mean.
+ * Up (field): r_fine(i) = 2 * trilinear(r_coarse, clamp(i/2 - 1/4)) per axis
+ * (cell-centre aligned), values doubled because the field is in voxel units.
+ * ---------------------------------------------------------------------- */
+void oracle_downsample(const float *v, int nx, int ny, int nz, float *out) {
+    int mx = nx / 2, my = ny / 2, mz = nz / 2;
+#pragma omp parallel for schedule(static)
+    for (int z = 0; z < mz; ++z)
+        for (int y = 0; y < my; ++y)
+            for (int x = 0; x < mx; ++x) {
+                double s = 0.0;
+                for (int c = 0; c < 2; ++c)
+                    for (int b = 0; b < 2; ++b)
+                        for (int a = 0; a < 2; ++a) s += v[IDX(2 * x + a, 2 * y + b, 2 * z + c)];
+                out[((size_t)z * my + y) * mx + x] = (float)(s / 8.0);
+            }
+}
+
+void oracle_upsample_field(const float *dc, int cx, int cy, int cz, float *out) {
+    int nx = 2 * cx, ny = 2 * cy, nz = 2 * cz;
+    size_t Nc = (size_t)cx * cy * cz, N = (size_t)nx * ny * nz;
+    for (int comp = 0; comp < 3; ++comp) {
+        const float *src = dc + comp * Nc;
+        float *dst = out + comp * N;
+#pragma omp parallel for schedule(static)
+        for (int z = 0; z < nz; ++z)
+            for (int y = 0; y < ny; ++y)
+                for (int x = 0; x < nx; ++x)
+                    dst[IDX(x, y, z)] = (float)(2.0 * trilinear(src, cx, cy, cz, x / 2.0 - 0.25, y / 2.0 - 0.25, z / 2.0 - 0.25));
+    }
+}
+
+/* ------------------------------------------------------------------------
+ * driver: Algorithm A1 minus the global shift (a no-op on
+ * this path, pin P8), minus step 2 (mask/interpolation, NEXT-1) and with a
+ * fixed iteration count instead of the while-test (reading A14).  Per level,
+ * `iters` x { warp, moments+correct, force+update, smooth }; up-sample r
+ * between levels; out_corr = correct(cbct_0, warp(ct_0, r)) (reading A12).
+ * The CBCT moments are those of the level's ORIGINAL cbct, so
+ * they are computed once per level with the same naive loop.
+ * `trace` (optional, may be NULL): receives sum|r| after every iteration.
+ * ---------------------------------------------------------------------- */
+void oracle_register(const float *ct, const float *cbct, int nx, int ny, int nz, int R, double sigma, int levels,
+                     int iters, double eps_var, double eps_den, float *out_disp, float *out_corr, double *trace) {
+    const float **pct = (const float **)malloc(sizeof(float *) * levels);
+    const float **pcb = (const float **)malloc(sizeof(float *) * levels);
+    pct[0] = ct; pcb[0] = cbct;
+    for (int l = 1; l < levels; ++l) {
+        int fx = nx >> (l - 1), fy = ny >> (l - 1), fz = nz >> (l - 1);
+        size_t Nl = (size_t)(fx / 2) * (fy / 2) * (fz / 2);
+        float *a = (float *)malloc(sizeof(float) * Nl), *b = (float *)malloc(sizeof(float) * Nl);
+        oracle_downsample(pct[l - 1], fx, fy, fz, a);
+        oracle_downsample(pcb[l - 1], fx, fy, fz, b);
+        pct[l] = a; pcb[l] = b;
+    }
+    float *r = NULL;
+    int it_total = 0;
+    for (int l = levels - 1; l >= 0; --l) {
+        int lx = nx >> l, ly = ny >> l, lz = nz >> l;
+        size_t N = (size_t)lx * ly * lz;
+        if (r == NULL) {
+            r = (float *)calloc(3 * N, sizeof(float));            /* PAPER.md:181 r = 0 */
+        } else {
+            float *rf = (float *)malloc(sizeof(float) * 3 * N);
+            oracle_upsample_field(r, lx / 2, ly / 2, lz / 2, rf);
+            free(r); r = rf;
+        }
+        float *m = (float *)malloc(sizeof(float) * N), *sp = (float *)malloc(sizeof(float) * N);
+        double *mus = (double *)malloc(sizeof(double) * N), *vs = (double *)malloc(sizeof(double) * N);
+        double *mum = (double *)malloc(sizeof(double) * N), *vm = (double *)malloc(sizeof(double) * N);
+        oracle_box_moments(pcb[l], lx, ly, lz, R, mus, vs);
+        for (int k = 0; k < iters; ++k) {
+            oracle_warp(pct[l], r, lx, ly, lz, m);                                   /* I_m^(k) */
+            oracle_box_moments(m, lx, ly, lz, R, mum, vm);                           /* A1 step 1 */
+            oracle_correct_from_moments(pcb[l], mus, vs, mum, vm, N, eps_var, sp);   /* A1 step 3 */
+            oracle_force_update(m, sp, lx, ly, lz, eps_den, r);                      /* A1 steps 4-5 */
+            oracle_smooth_field(r, lx, ly, lz, sigma);                               /* A1 step 6 */
+            if (trace) {
+                double s = 0.0;
+                for (size_t i = 0; i < 3 * N; ++i) s += fabs((double)r[i]);
+                trace[it_total] = s;
+            }
+            ++it_total;
+        }
+        if (l == 0) {
+            memcpy(out_disp, r, sizeof(float) * 3 * N);
+            if (out_corr) {
+                oracle_warp(pct[0], r, lx, ly, lz, m);
+                oracle_box_moments(m, lx, ly, lz, R, mum, vm);
+                oracle_correct_from_moments(pcb[0], mus, vs, mum, vm, N, eps_var, out_corr);
+            }
+        }
+        free(m); free(sp); free(mus); free(vs); free(mum); free(vm);
+    }
+    free(r);
+    for (int l = 1; l < levels; ++l) { free((void *)pct[l]); free((void *)pcb[l]); }
+    free(pct); free(pcb);
+}
