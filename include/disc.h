@@ -1,0 +1,144 @@
+/*
+ * disc.h -- C-ABI of the B200-native DISC hot path (CT -> CBCT demons registration with
+ * simultaneous patch-moment intensity correction; Zhen et al., arxiv 1204.6295).
+ * Citations are PAPER.md:LINE of that paper's text; "reading Ax" refers to DESIGN.md.
+ *
+ * Plain C: no C++ types, no exceptions, no torch types.  One GPU (sm_100a), one context per
+ * stream at a time.  Nothing here runs on the CPU: without a CUDA device every compute call
+ * returns DISC_ERR_CUDA / DISC_ERR_UNSUPPORTED -- there is no fallback.
+ *
+ * Conventions
+ *   dims = (nx, ny, nz), x fastest: idx = (z*ny + y)*nx + x.  All volumes are float32.
+ *   A displacement field is planar: disp[c*N + idx], c = 0,1,2 <-> x,y,z, in VOXEL units of the
+ *   level it lives on (reading A13).  Level 0 is the finest; level l has dims >> l.
+ *   The moving image is the CT, the static image the CBCT.  The field is a
+ *   pull-back: warped(x) = ct(x + r(x)), so for cbct(x) = ct(x + u(x)) the
+ *   registration returns r ~ u (reading A1).
+ *   Unless a parameter says HOST, every pointer is a DEVICE pointer owned by the caller; the
+ *   library never frees or keeps it after the call's work has run.  Inputs are never written.
+ *   Outputs must not alias inputs except where a parameter is named *_inout.
+ *   `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Every call only
+ *   enqueues work on it and returns; the library never synchronises (except disc_destroy and
+ *   disc_register_host, which say so).  Scratch lives in the context, so one context must not
+ *   be used from two streams concurrently.
+ *   Errors: argument errors are detected before any launch and return DISC_ERR_INVALID_ARG;
+ *   launch/runtime failures return DISC_ERR_CUDA; disc_last_error() gives a message.
+ */
+#ifndef DISC_H
+#define DISC_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct disc_ctx disc_ctx; /* opaque, owned by the library */
+
+typedef enum {
+    DISC_OK = 0,
+    DISC_ERR_INVALID_ARG = 1,
+    DISC_ERR_UNSUPPORTED = 2, /* no sm_100 device, patch_radius > 10, Gaussian radius > 12 */
+    DISC_ERR_ALLOC = 3,
+    DISC_ERR_CUDA = 4
+} disc_status;
+
+/* Limits of this build. */
+#define DISC_MAX_PATCH_RADIUS 10
+#define DISC_MAX_GAUSS_RADIUS 12 /* ceil(3*sigma) <= 12, i.e. sigma <= 4 */
+#define DISC_MAX_LEVELS 8
+
+/* Regularisers (readings A5, A7): a = 0 where var_s <= DISC_EPS_VAR [HU^2];
+ * force denominator |g|^2 + d^2 + DISC_EPS_DEN [HU^2]. */
+#define DISC_EPS_VAR 1e-6f
+#define DISC_EPS_DEN 1e-3f
+
+/*
+ * disc_create -- problem statement of the paper (Alg. A1 :175-198).
+ *   dims          (nx, ny, nz) of level 0, each >= 1 and divisible by 2^(levels-1).   HOST
+ *   spacing       voxel size in mm, each > 0.  Validated and stored; the hot path works in voxel
+ *                 units (Eq. (1) has no spacing term; reading A13).          HOST
+ *   patch_radius  R >= 0; the patch is the cube of side 2R+1 truncated to the volume (PAPER.md:87-89,
+ *                 reading A4), the same R in voxels at every level.
+ *   sigma_smooth  Gaussian sigma in voxels, > 0; support K = ceil(3 sigma), replicate border (A10).
+ *   levels        pyramid levels >= 1, factor 2 per level in all three axes (A9).
+ *   iters         iterations per level >= 0 (fixed count instead of the stopping test, A14).
+ * Allocates all scratch (pyramid copies, warped CT, corrected CBCT, cached CBCT patch z-score,
+ * second field buffer) on the current CUDA device.  Returns DISC_ERR_UNSUPPORTED if the current
+ * device is not compute capability 10.x.
+ */
+disc_status disc_create(disc_ctx** out, const int dims[3], const float spacing[3], int patch_radius,
+                        float sigma_smooth, int levels, int iters);
+
+/* Synchronises the device, frees the context and its scratch.  NULL is allowed. */
+void disc_destroy(disc_ctx* ctx);
+
+/* Message of the last error of this context (or of the last failed disc_create when ctx == NULL).
+ * The string is owned by the library and valid until the next call on the same context. */
+const char* disc_last_error(const disc_ctx* ctx);
+
+/* Number of CUDA kernels this context has launched so far (bench.py's gpu_launches). */
+unsigned long long disc_launch_count(const disc_ctx* ctx);
+
+/* ---- the steps of one iteration, in execution order b -> a -> c+d (Alg. A1) ---- */
+
+/* (b) out(x) = moving(x + disp(x)), trilinear, sample position clamped to the volume
+ * ("update the moving image", kernel 5 :171; reading A11).
+ * moving [N_level], disp [3*N_level], out [N_level]. */
+disc_status disc_warp(disc_ctx* ctx, int level, const float* moving, const float* disp, float* out, void* stream);
+
+/* (a) out = a*(cbct - mu_cbct) + mu_ct with a = STD(ct patch)/STD(cbct patch), patch moments over
+ * the truncated cube of radius R (PAPER.md:95 Eq. 3, :117-119 Eqs. 5-6, :141; readings A4, A5):
+ * a = 0 where var_cbct <= DISC_EPS_VAR.  cbct, ct_warped, out_corrected: [N_level]. */
+disc_status disc_correct_intensity(disc_ctx* ctx, int level, const float* cbct, const float* ct_warped,
+                                   float* out_corrected, void* stream);
+
+/* (c)+(d) = Alg. A1 steps 4-6: disp += (s-m) grad s / (|grad s|^2 + (s-m)^2 + eps)
+ * (Eq. 1 first term; readings A1, A2, A7, A8), then disp <- G_sigma * disp (A3, A10).
+ * m_warped, s_corrected: [N_level]; disp_inout: [3*N_level], updated in place. */
+disc_status disc_demons_step(disc_ctx* ctx, int level, const float* m_warped, const float* s_corrected,
+                             float* disp_inout, void* stream);
+
+/* The whole registration (Alg. A1, fixed `iters` per level): builds both pyramids
+ * (2x2x2 means), r = 0 at the coarsest level, per level `iters` x {warp, correct, force+update,
+ * smooth}, up-samples r between levels (x2 trilinear, values doubled), and finally
+ * out_corrected_cbct = correct(cbct, warp(ct, out_disp)) (reading A12).
+ * ct, cbct: [N_0]; out_disp: [3*N_0]; out_corrected_cbct: [N_0] or NULL. */
+disc_status disc_register(disc_ctx* ctx, const float* ct, const float* cbct, float* out_disp,
+                          float* out_corrected_cbct, void* stream);
+
+/* Same as disc_register with HOST buffers (pageable or pinned): copies ct and cbct to the device,
+ * registers, copies the results back and SYNCHRONISES `stream` before returning.
+ * This is the end-to-end entry point bench.py times ("e2e"). */
+disc_status disc_register_host(disc_ctx* ctx, const float* ct_host, const float* cbct_host, float* out_disp_host,
+                               float* out_corrected_cbct_host, void* stream);
+
+/* `n_iters` iterations of {correct, force+update, smooth, warp} at one level, starting from
+ * disp_inout (the fused steady-state loop of disc_register; what bench.py times as iterations/s).
+ * ct, cbct: [N_level] images of that level; disp_inout [3*N_level].  After the call the context's
+ * warped-CT buffer holds warp(ct, disp_inout). */
+disc_status disc_iterate(disc_ctx* ctx, int level, const float* ct, const float* cbct, float* disp_inout,
+                         int n_iters, void* stream);
+
+/* ---- finer-grained exports (BASELINE.json config 5 per-kernel sweep, and tests) ---- */
+
+/* Patch mean and population variance of `vol` over the truncated cube of radius R (Eq. 3, A4).
+ * mean, var: [N_level] float32. */
+disc_status disc_box_moments(disc_ctx* ctx, int level, const float* vol, float* mean, float* var, void* stream);
+
+/* Step (c) alone: disp_inout += force(m, s). */
+disc_status disc_force_update(disc_ctx* ctx, int level, const float* m, const float* s, float* disp_inout, void* stream);
+
+/* Step (d) alone: disp_inout <- G_sigma * disp_inout. */
+disc_status disc_smooth_field(disc_ctx* ctx, int level, float* disp_inout, void* stream);
+
+/* 2x2x2 block mean from level_from to level_from+1 (reading A9).
+ * vol [N_level_from], out [N_level_from / 8]. */
+disc_status disc_downsample(disc_ctx* ctx, int level_from, const float* vol, float* out, void* stream);
+
+/* x2 trilinear up-sampling of a field from level_from to level_from-1 at i/2 - 1/4 (clamped), values
+ * doubled (reading A9).  disp [3*N_level_from], out [3*8*N_level_from]. */
+disc_status disc_upsample_field(disc_ctx* ctx, int level_from, const float* disp, float* out, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DISC_H */

@@ -1,0 +1,210 @@
+"""Python binding of the DISC C-ABI (`include/disc.h`): argument marshalling only.
+
+Every function has the name and argument order of its C counterpart and does nothing but check tensor
+device / dtype / contiguity / size and pass `data_ptr()` and the current CUDA stream.  Every step of the path
+runs in the CUDA kernels of `libdisc.so`; there is no CPU or PyTorch fallback -- if the library is missing the
+import fails, and without a B200 `disc_create` raises.
+
+PyTorch is used for device memory and streams only.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdisc.so")
+
+DISC_OK, DISC_ERR_INVALID_ARG, DISC_ERR_UNSUPPORTED, DISC_ERR_ALLOC, DISC_ERR_CUDA = range(5)
+DISC_MAX_PATCH_RADIUS = 10
+DISC_MAX_GAUSS_RADIUS = 12
+DISC_EPS_VAR = 1e-6
+DISC_EPS_DEN = 1e-3
+
+EXPORTS = (
+    "disc_create", "disc_destroy", "disc_last_error", "disc_launch_count", "disc_warp", "disc_correct_intensity",
+    "disc_demons_step", "disc_register", "disc_register_host", "disc_iterate", "disc_box_moments",
+    "disc_force_update", "disc_smooth_field", "disc_downsample", "disc_upsample_field",
+)
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} is missing: build it with `python -m paper_1204_6295_b200.build` "
+        "(or `__graft_entry__.build()`); there is no fallback path")
+
+_lib = ctypes.CDLL(LIB_PATH)
+_vp, _i = ctypes.c_void_p, ctypes.c_int
+_lib.disc_create.restype = _i
+_lib.disc_create.argtypes = [ctypes.POINTER(_vp), ctypes.POINTER(_i), ctypes.POINTER(ctypes.c_float), _i,
+                             ctypes.c_float, _i, _i]
+_lib.disc_destroy.restype = None
+_lib.disc_destroy.argtypes = [_vp]
+_lib.disc_last_error.restype = ctypes.c_char_p
+_lib.disc_last_error.argtypes = [_vp]
+_lib.disc_launch_count.restype = ctypes.c_ulonglong
+_lib.disc_launch_count.argtypes = [_vp]
+for _name, _nptr in (("disc_warp", 3), ("disc_correct_intensity", 3), ("disc_demons_step", 3),
+                     ("disc_box_moments", 3), ("disc_force_update", 3), ("disc_smooth_field", 1),
+                     ("disc_downsample", 2), ("disc_upsample_field", 2)):
+    _f = getattr(_lib, _name)
+    _f.restype = _i
+    _f.argtypes = [_vp, _i] + [_vp] * _nptr + [_vp]
+_lib.disc_register.restype = _i
+_lib.disc_register.argtypes = [_vp] * 6
+_lib.disc_register_host.restype = _i
+_lib.disc_register_host.argtypes = [_vp] * 6
+_lib.disc_iterate.restype = _i
+_lib.disc_iterate.argtypes = [_vp, _i, _vp, _vp, _vp, _i, _vp]
+
+
+class DiscError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__(f"disc status {status}: {message}")
+        self.status = status
+
+
+def _check(ctx, status):
+    if status != DISC_OK:
+        msg = _lib.disc_last_error(ctx)
+        raise DiscError(status, msg.decode() if msg else "")
+
+
+def _dev(t, numel=None):
+    """device pointer of a CUDA float32 contiguous tensor (None -> NULL)"""
+    if t is None:
+        return None
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise TypeError("expected a contiguous float32 CUDA tensor")
+    if numel is not None and t.numel() != int(numel):
+        raise ValueError(f"tensor has {t.numel()} elements, expected {numel}")
+    return t.data_ptr()
+
+
+def _x3(n):
+    return None if n is None else 3 * n
+
+
+def _host(a):
+    """host pointer of a float32 C-contiguous numpy array or CPU tensor (None -> NULL)"""
+    if a is None:
+        return None
+    if hasattr(a, "data_ptr"):
+        if a.is_cuda or not a.is_contiguous() or a.element_size() != 4:
+            raise TypeError("expected a contiguous float32 CPU tensor")
+        return a.data_ptr()
+    if a.dtype.itemsize != 4 or not a.flags["C_CONTIGUOUS"]:
+        raise TypeError("expected a C-contiguous float32 numpy array")
+    return a.ctypes.data
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+class Ctx:
+    """Opaque handle returned by disc_create (keeps the level sizes for argument checks)."""
+
+    def __init__(self, handle, dims, levels):
+        self.handle = handle
+        self.dims = tuple(dims)
+        self.levels = levels
+
+    def n(self, level):
+        """voxels at `level`; None for a level the context does not have (the C layer reports that)"""
+        if not 0 <= level < self.levels:
+            return None
+        nx, ny, nz = self.dims
+        return (nx >> level) * (ny >> level) * (nz >> level)
+
+    def __del__(self):
+        h, self.handle = getattr(self, "handle", None), None
+        if h:
+            _lib.disc_destroy(h)
+
+
+def disc_create(dims, spacing, patch_radius, sigma_smooth, levels, iters) -> Ctx:
+    out = _vp()
+    d = (_i * 3)(*[int(v) for v in dims])
+    s = (ctypes.c_float * 3)(*[float(v) for v in spacing])
+    st = _lib.disc_create(ctypes.byref(out), d, s, int(patch_radius), float(sigma_smooth), int(levels), int(iters))
+    _check(None, st)
+    return Ctx(out.value, dims, levels)
+
+
+def disc_destroy(ctx: Ctx) -> None:
+    h, ctx.handle = ctx.handle, None
+    if h:
+        _lib.disc_destroy(h)
+
+
+def disc_last_error(ctx: Ctx | None) -> str:
+    msg = _lib.disc_last_error(ctx.handle if ctx else None)
+    return msg.decode() if msg else ""
+
+
+def disc_launch_count(ctx: Ctx) -> int:
+    return int(_lib.disc_launch_count(ctx.handle))
+
+
+def disc_warp(ctx, level, moving, disp, out, stream=None):
+    n = ctx.n(level)
+    _check(ctx.handle, _lib.disc_warp(ctx.handle, level, _dev(moving, n), _dev(disp, _x3(n)), _dev(out, n), _stream(stream)))
+
+
+def disc_correct_intensity(ctx, level, cbct, ct_warped, out_corrected, stream=None):
+    n = ctx.n(level)
+    _check(ctx.handle, _lib.disc_correct_intensity(ctx.handle, level, _dev(cbct, n), _dev(ct_warped, n),
+                                                   _dev(out_corrected, n), _stream(stream)))
+
+
+def disc_demons_step(ctx, level, m_warped, s_corrected, disp_inout, stream=None):
+    n = ctx.n(level)
+    _check(ctx.handle, _lib.disc_demons_step(ctx.handle, level, _dev(m_warped, n), _dev(s_corrected, n),
+                                             _dev(disp_inout, _x3(n)), _stream(stream)))
+
+
+def disc_register(ctx, ct, cbct, out_disp, out_corrected_cbct, stream=None):
+    n = ctx.n(0)
+    _check(ctx.handle, _lib.disc_register(ctx.handle, _dev(ct, n), _dev(cbct, n), _dev(out_disp, _x3(n)),
+                                          _dev(out_corrected_cbct, n), _stream(stream)))
+
+
+def disc_register_host(ctx, ct_host, cbct_host, out_disp_host, out_corrected_cbct_host, stream=None):
+    _check(ctx.handle, _lib.disc_register_host(ctx.handle, _host(ct_host), _host(cbct_host), _host(out_disp_host),
+                                               _host(out_corrected_cbct_host), _stream(stream)))
+
+
+def disc_iterate(ctx, level, ct, cbct, disp_inout, n_iters, stream=None):
+    n = ctx.n(level)
+    _check(ctx.handle, _lib.disc_iterate(ctx.handle, level, _dev(ct, n), _dev(cbct, n), _dev(disp_inout, _x3(n)),
+                                         int(n_iters), _stream(stream)))
+
+
+def disc_box_moments(ctx, level, vol, mean, var, stream=None):
+    n = ctx.n(level)
+    _check(ctx.handle, _lib.disc_box_moments(ctx.handle, level, _dev(vol, n), _dev(mean, n), _dev(var, n), _stream(stream)))
+
+
+def disc_force_update(ctx, level, m, s, disp_inout, stream=None):
+    n = ctx.n(level)
+    _check(ctx.handle, _lib.disc_force_update(ctx.handle, level, _dev(m, n), _dev(s, n), _dev(disp_inout, _x3(n)),
+                                              _stream(stream)))
+
+
+def disc_smooth_field(ctx, level, disp_inout, stream=None):
+    n = ctx.n(level)
+    _check(ctx.handle, _lib.disc_smooth_field(ctx.handle, level, _dev(disp_inout, _x3(n)), _stream(stream)))
+
+
+def disc_downsample(ctx, level_from, vol, out, stream=None):
+    _check(ctx.handle, _lib.disc_downsample(ctx.handle, level_from, _dev(vol, ctx.n(level_from)),
+                                            _dev(out, ctx.n(level_from + 1)), _stream(stream)))
+
+
+def disc_upsample_field(ctx, level_from, disp, out, stream=None):
+    _check(ctx.handle, _lib.disc_upsample_field(ctx.handle, level_from, _dev(disp, _x3(ctx.n(level_from))),
+                                                _dev(out, _x3(ctx.n(level_from - 1))), _stream(stream)))

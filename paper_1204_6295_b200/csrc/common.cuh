@@ -1,0 +1,48 @@
+// common.cuh -- small device helpers shared by the DISC kernels (sm_100a).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace disc {
+
+constexpr int kMaxGaussTaps = 2 * 12 + 1;
+
+// Gaussian taps travel as a kernel parameter (constant bank): FFMA reads them as immediates-from-bank.
+struct GaussTaps {
+    float w[kMaxGaussTaps];
+};
+
+struct Dims {
+    int nx, ny, nz;
+};
+
+__device__ __forceinline__ int clampi(int v, int lo, int hi) { return min(max(v, lo), hi); }
+
+// Trilinear sample of I at (px,py,pz), position clamped to the volume (reading A11):
+// p = clamp(p, 0, n-1), i0 = min(floor(p), n-2), t = p - i0; an axis of length 1 has weight 0.
+__device__ __forceinline__ float trilinear_clamped(const float* __restrict__ I, int nx, int ny, int nz, float px,
+                                                   float py, float pz) {
+    px = fminf(fmaxf(px, 0.f), (float)(nx - 1));
+    py = fminf(fmaxf(py, 0.f), (float)(ny - 1));
+    pz = fminf(fmaxf(pz, 0.f), (float)(nz - 1));
+    const int x0 = max(min((int)px, nx - 2), 0), y0 = max(min((int)py, ny - 2), 0), z0 = max(min((int)pz, nz - 2), 0);
+    const int dx = nx > 1 ? 1 : 0;
+    const size_t dy = ny > 1 ? (size_t)nx : 0, dz = nz > 1 ? (size_t)nx * ny : 0;
+    const float tx = px - (float)x0, ty = py - (float)y0, tz = pz - (float)z0;
+    const float* p = I + ((size_t)z0 * ny + y0) * nx + x0;
+    const float a000 = __ldg(p), a100 = __ldg(p + dx);
+    const float a010 = __ldg(p + dy), a110 = __ldg(p + dy + dx);
+    const float a001 = __ldg(p + dz), a101 = __ldg(p + dz + dx);
+    const float a011 = __ldg(p + dz + dy), a111 = __ldg(p + dz + dy + dx);
+    // (1-t)*a + t*b: exact at t = 0 and t = 1, so a zero field reproduces the input bit for bit
+    const float ux = 1.f - tx, uy = 1.f - ty, uz = 1.f - tz;
+    const float c00 = fmaf(tx, a100, ux * a000);
+    const float c10 = fmaf(tx, a110, ux * a010);
+    const float c01 = fmaf(tx, a101, ux * a001);
+    const float c11 = fmaf(tx, a111, ux * a011);
+    const float c0 = fmaf(ty, c10, uy * c00);
+    const float c1 = fmaf(ty, c11, uy * c01);
+    return fmaf(tz, c1, uz * c0);
+}
+
+}  // namespace disc

@@ -1,0 +1,387 @@
+// disc_api.cu -- context, argument validation, launch plumbing and the extern "C" boundary of
+// include/disc.h.  Every step of the path runs in the kernels of moments.cuh / field.cuh / pyramid.cuh;
+// this file only sizes grids, picks template instances and enqueues launches on the caller's stream.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/disc.h"
+#include "launch.h"
+#include "pyramid.cuh"
+
+using namespace disc;
+
+namespace {
+
+struct Level {
+    int nx, ny, nz;
+    size_t N;
+    float* ct;       // pyramid copy (levels >= 1); level 0 uses the caller's pointer
+    float* cbct;     // idem
+    float* zhat;     // cached CBCT patch z-score (I_s - mu_s)/sigma_s of this level   [N]
+    float* m;        // warped CT                                                        [N]
+    float* sp;       // corrected CBCT                                                   [N]
+    float* disp;     // field of this level (levels >= 1; level 0 uses the caller's)     [3N]
+    float* scratch;  // field after the x,y Gaussian passes                              [3N]
+};
+
+thread_local char g_create_error[256] = "";
+
+}  // namespace
+
+struct disc_ctx {
+    int dims[3];
+    float spacing[3];
+    int R;
+    float sigma;
+    int levels, iters;
+    int K;
+    GaussTaps taps;
+    Level lv[DISC_MAX_LEVELS];
+    float* h2d_ct;    // device staging for disc_register_host
+    float* h2d_cbct;
+    float* d_out_disp;
+    float* d_out_corr;
+    unsigned long long launches;
+    char err[256];
+};
+
+namespace {
+
+disc_status fail(disc_ctx* c, disc_status st, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(c ? c->err : g_create_error, 256, fmt, ap);
+    va_end(ap);
+    return st;
+}
+
+disc_status check_launch(disc_ctx* c, const char* what) {
+    c->launches++;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(c, DISC_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+    return DISC_OK;
+}
+
+#define DISC_TRY(expr)                         \
+    do {                                       \
+        disc_status _s = (expr);               \
+        if (_s != DISC_OK) return _s;          \
+    } while (0)
+
+#define DISC_NEED(c, cond, msg)                                             \
+    do {                                                                    \
+        if (!(cond)) return fail((c), DISC_ERR_INVALID_ARG, "%s", (msg));   \
+    } while (0)
+
+bool level_ok(const disc_ctx* c, int level) { return level >= 0 && level < c->levels; }
+
+int pick_chunk(int n, int min_chunk, long long ctas_per_chunk, long long target_ctas) {
+    // split an axis of length n into chunks so that the grid reaches ~target_ctas CTAs,
+    // but never below min_chunk (each chunk re-reads a halo)
+    long long want = target_ctas / ctas_per_chunk;  // round down: prefer one full wave over 1.x waves
+    if (want < 1) want = 1;
+    int chunk = (int)((n + want - 1) / want);
+    if (chunk < min_chunk) chunk = min_chunk;
+    if (chunk > n) chunk = n;
+    return chunk;
+}
+
+// ------------------------------------------------------------------ kernels instantiated in moments_tu.cu / field_tu.cu
+template <int MODE>
+disc_status launch_moments(disc_ctx* c, const Level& L, const float* vol, const float* aux, float* out0,
+                           float* out1, cudaStream_t st) {
+    const int tiles = ((L.nx + kMomTX - 1) / kMomTX) * ((L.ny + kMomTY - 1) / kMomTY);
+    const int W = 2 * c->R + 1;
+    const int zchunk = pick_chunk(L.nz, 4 * W > 32 ? 4 * W : 32, tiles, 2 * 148);
+    if (!launch_moments_any(c->R, MODE, vol, aux, out0, out1, L.nx, L.ny, L.nz, zchunk, DISC_EPS_VAR, st))
+        return fail(c, DISC_ERR_UNSUPPORTED, "patch_radius %d > %d", c->R, DISC_MAX_PATCH_RADIUS);
+    return check_launch(c, "k_moments");
+}
+
+template <bool FORCE>
+disc_status launch_force_gxy(disc_ctx* c, const Level& L, const float* m, const float* s, const float* rin,
+                             float* rout, cudaStream_t st) {
+    const int txb = L.nx > 64 ? 128 : (L.nx > 32 ? 64 : 32);
+    const int xt = (L.nx + txb - 1) / txb;
+    const int K = c->K;
+    const int yseg = pick_chunk(L.ny, 8 * K > 32 ? 8 * K : 32, (long long)xt * L.nz, 4 * 148);
+    if (!launch_force_gxy_any(K, FORCE, txb, m, s, rin, rout, L.nx, L.ny, L.nz, yseg, DISC_EPS_DEN, c->taps, st))
+        return fail(c, DISC_ERR_UNSUPPORTED, "Gaussian radius %d unsupported", K);
+    return check_launch(c, "k_force_gxy");
+}
+
+template <bool WARP>
+disc_status launch_gz_warp(disc_ctx* c, const Level& L, const float* rin, float* rout, const float* moving,
+                           float* mout, cudaStream_t st) {
+    const size_t plane = (size_t)L.nx * L.ny;
+    const int bx = (int)((plane + 127) / 128);
+    const int K = c->K;
+    const int zchunk = pick_chunk(L.nz, 8 * K > 32 ? 8 * K : 32, bx, 8 * 148);
+    if (!launch_gz_warp_any(K, WARP, rin, rout, moving, mout, L.nx, L.ny, L.nz, zchunk, c->taps, st))
+        return fail(c, DISC_ERR_UNSUPPORTED, "Gaussian radius %d unsupported", K);
+    return check_launch(c, "k_gz_warp");
+}
+
+disc_status launch_warp(disc_ctx* c, const Level& L, const float* moving, const float* r, float* out, cudaStream_t st) {
+    launch_warp_kernel(moving, r, out, L.nx, L.ny, L.nz, st);
+    return check_launch(c, "k_warp");
+}
+
+disc_status launch_downsample(disc_ctx* c, const Level& fine, const float* in, float* out, cudaStream_t st) {
+    const int mx = fine.nx / 2, my = fine.ny / 2, mz = fine.nz / 2;
+    dim3 grid((mx + 127) / 128, my, mz);
+    k_downsample<<<grid, 128, 0, st>>>(in, out, mx, my, mz);
+    return check_launch(c, "k_downsample");
+}
+
+disc_status launch_upsample(disc_ctx* c, const Level& coarse, const float* in, float* out, cudaStream_t st) {
+    const int nx = 2 * coarse.nx, ny = 2 * coarse.ny, nz = 2 * coarse.nz;
+    dim3 grid((nx + 127) / 128, ny, 3 * nz);
+    k_upsample_field<<<grid, 128, 0, st>>>(in, out, coarse.nx, coarse.ny, coarse.nz);
+    return check_launch(c, "k_upsample_field");
+}
+
+// n_iters x { correct, force+update+Gxy, Gz+warp } on level L; on entry L.m must hold warp(ct, disp).
+// With final_warp the last iteration also refreshes L.m (needed when the caller goes on using it).
+disc_status iterate_level(disc_ctx* c, Level& L, const float* ct, float* disp, int n_iters, bool final_warp,
+                          cudaStream_t st) {
+    for (int k = 0; k < n_iters; ++k) {
+        DISC_TRY(launch_moments<kModeCorrect>(c, L, L.m, L.zhat, L.sp, nullptr, st));       // A1 steps 1,3
+        DISC_TRY(launch_force_gxy<true>(c, L, L.m, L.sp, disp, L.scratch, st));              // A1 steps 4,5,6(x,y)
+        if (k + 1 < n_iters || final_warp)
+            DISC_TRY(launch_gz_warp<true>(c, L, L.scratch, disp, ct, L.m, st));              // A1 step 6(z) + next I_m^(k)
+        else
+            DISC_TRY(launch_gz_warp<false>(c, L, L.scratch, disp, nullptr, nullptr, st));
+    }
+    return DISC_OK;
+}
+
+void free_ctx(disc_ctx* c) {
+    for (int l = 0; l < DISC_MAX_LEVELS; ++l) {
+        Level& L = c->lv[l];
+        cudaFree(L.ct); cudaFree(L.cbct); cudaFree(L.zhat); cudaFree(L.m); cudaFree(L.sp);
+        cudaFree(L.disp); cudaFree(L.scratch);
+    }
+    cudaFree(c->h2d_ct); cudaFree(c->h2d_cbct); cudaFree(c->d_out_disp); cudaFree(c->d_out_corr);
+    delete c;
+}
+
+}  // namespace
+
+// =====================================================================================
+extern "C" {
+
+disc_status disc_create(disc_ctx** out, const int dims[3], const float spacing[3], int patch_radius,
+                        float sigma_smooth, int levels, int iters) {
+    if (!out) return fail(nullptr, DISC_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (!dims || !spacing) return fail(nullptr, DISC_ERR_INVALID_ARG, "dims/spacing is NULL");
+    if (levels < 1 || levels > DISC_MAX_LEVELS) return fail(nullptr, DISC_ERR_INVALID_ARG, "levels must be in 1..%d", DISC_MAX_LEVELS);
+    for (int i = 0; i < 3; ++i) {
+        if (dims[i] < 1) return fail(nullptr, DISC_ERR_INVALID_ARG, "dims[%d] < 1", i);
+        if (!(spacing[i] > 0.f)) return fail(nullptr, DISC_ERR_INVALID_ARG, "spacing[%d] <= 0", i);
+        if (dims[i] % (1 << (levels - 1)) != 0)
+            return fail(nullptr, DISC_ERR_INVALID_ARG, "dims[%d]=%d not divisible by 2^(levels-1)", i, dims[i]);
+    }
+    if (patch_radius < 0) return fail(nullptr, DISC_ERR_INVALID_ARG, "patch_radius < 0");
+    if (!(sigma_smooth > 0.f)) return fail(nullptr, DISC_ERR_INVALID_ARG, "sigma_smooth <= 0");
+    if (iters < 0) return fail(nullptr, DISC_ERR_INVALID_ARG, "iters < 0");
+    if (patch_radius > DISC_MAX_PATCH_RADIUS)
+        return fail(nullptr, DISC_ERR_UNSUPPORTED, "patch_radius %d > %d", patch_radius, DISC_MAX_PATCH_RADIUS);
+    const int K = (int)std::ceil(3.0 * (double)sigma_smooth);
+    if (K > DISC_MAX_GAUSS_RADIUS)
+        return fail(nullptr, DISC_ERR_UNSUPPORTED, "Gaussian radius ceil(3 sigma) = %d > %d", K, DISC_MAX_GAUSS_RADIUS);
+
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(nullptr, DISC_ERR_CUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+    int major = 0;
+    e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) return fail(nullptr, DISC_ERR_CUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e));
+    if (major != 10) return fail(nullptr, DISC_ERR_UNSUPPORTED, "device compute capability %d.x, this library is sm_100a only", major);
+
+    disc_ctx* c = new (std::nothrow) disc_ctx();
+    if (!c) return fail(nullptr, DISC_ERR_ALLOC, "out of host memory");
+    std::memset(c, 0, sizeof(*c));
+    for (int i = 0; i < 3; ++i) { c->dims[i] = dims[i]; c->spacing[i] = spacing[i]; }
+    c->R = patch_radius; c->sigma = sigma_smooth; c->levels = levels; c->iters = iters; c->K = K;
+    // Gaussian taps: fp64, normalised to sum 1, then rounded to fp32 (reading A10)
+    {
+        double w[kMaxGaussTaps], sum = 0.0;
+        for (int i = -K; i <= K; ++i) { w[i + K] = std::exp(-(double)(i * i) / (2.0 * (double)sigma_smooth * (double)sigma_smooth)); sum += w[i + K]; }
+        for (int i = 0; i < 2 * K + 1; ++i) c->taps.w[i] = (float)(w[i] / sum);
+    }
+    for (int l = 0; l < levels; ++l) {
+        Level& L = c->lv[l];
+        L.nx = dims[0] >> l; L.ny = dims[1] >> l; L.nz = dims[2] >> l;
+        L.N = (size_t)L.nx * L.ny * L.nz;
+        const size_t b = L.N * sizeof(float);
+        bool ok = cudaMalloc(&L.zhat, b) == cudaSuccess && cudaMalloc(&L.m, b) == cudaSuccess &&
+                  cudaMalloc(&L.sp, b) == cudaSuccess && cudaMalloc(&L.scratch, 3 * b) == cudaSuccess;
+        if (ok && l > 0)
+            ok = cudaMalloc(&L.ct, b) == cudaSuccess && cudaMalloc(&L.cbct, b) == cudaSuccess &&
+                 cudaMalloc(&L.disp, 3 * b) == cudaSuccess;
+        if (!ok) {
+            cudaGetLastError();
+            free_ctx(c);
+            return fail(nullptr, DISC_ERR_ALLOC, "cudaMalloc failed at level %d", l);
+        }
+    }
+    *out = c;
+    return DISC_OK;
+}
+
+void disc_destroy(disc_ctx* ctx) {
+    if (!ctx) return;
+    cudaDeviceSynchronize();
+    free_ctx(ctx);
+}
+
+const char* disc_last_error(const disc_ctx* ctx) { return ctx ? ctx->err : g_create_error; }
+
+unsigned long long disc_launch_count(const disc_ctx* ctx) { return ctx ? ctx->launches : 0ull; }
+
+disc_status disc_warp(disc_ctx* c, int level, const float* moving, const float* disp, float* out, void* stream) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_NEED(c, level_ok(c, level), "level out of range");
+    DISC_NEED(c, moving && disp && out, "NULL pointer");
+    return launch_warp(c, c->lv[level], moving, disp, out, (cudaStream_t)stream);
+}
+
+disc_status disc_correct_intensity(disc_ctx* c, int level, const float* cbct, const float* ct_warped,
+                                   float* out_corrected, void* stream) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_NEED(c, level_ok(c, level), "level out of range");
+    DISC_NEED(c, cbct && ct_warped && out_corrected, "NULL pointer");
+    Level& L = c->lv[level];
+    cudaStream_t st = (cudaStream_t)stream;
+    DISC_TRY(launch_moments<kModeZscore>(c, L, cbct, nullptr, L.zhat, nullptr, st));
+    return launch_moments<kModeCorrect>(c, L, ct_warped, L.zhat, out_corrected, nullptr, st);
+}
+
+disc_status disc_demons_step(disc_ctx* c, int level, const float* m_warped, const float* s_corrected,
+                             float* disp_inout, void* stream) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_NEED(c, level_ok(c, level), "level out of range");
+    DISC_NEED(c, m_warped && s_corrected && disp_inout, "NULL pointer");
+    Level& L = c->lv[level];
+    cudaStream_t st = (cudaStream_t)stream;
+    DISC_TRY(launch_force_gxy<true>(c, L, m_warped, s_corrected, disp_inout, L.scratch, st));
+    return launch_gz_warp<false>(c, L, L.scratch, disp_inout, nullptr, nullptr, st);
+}
+
+disc_status disc_iterate(disc_ctx* c, int level, const float* ct, const float* cbct, float* disp_inout,
+                         int n_iters, void* stream) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_NEED(c, level_ok(c, level), "level out of range");
+    DISC_NEED(c, ct && cbct && disp_inout, "NULL pointer");
+    DISC_NEED(c, n_iters >= 0, "n_iters < 0");
+    Level& L = c->lv[level];
+    cudaStream_t st = (cudaStream_t)stream;
+    DISC_TRY(launch_moments<kModeZscore>(c, L, cbct, nullptr, L.zhat, nullptr, st));
+    DISC_TRY(launch_warp(c, L, ct, disp_inout, L.m, st));
+    return iterate_level(c, L, ct, disp_inout, n_iters, true, st);
+}
+
+disc_status disc_register(disc_ctx* c, const float* ct, const float* cbct, float* out_disp,
+                          float* out_corrected_cbct, void* stream) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_NEED(c, ct && cbct && out_disp, "NULL pointer");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int nl = c->levels;
+    // pyramids
+    const float* pct[DISC_MAX_LEVELS];
+    const float* pcb[DISC_MAX_LEVELS];
+    pct[0] = ct; pcb[0] = cbct;
+    for (int l = 1; l < nl; ++l) {
+        DISC_TRY(launch_downsample(c, c->lv[l - 1], pct[l - 1], c->lv[l].ct, st));
+        DISC_TRY(launch_downsample(c, c->lv[l - 1], pcb[l - 1], c->lv[l].cbct, st));
+        pct[l] = c->lv[l].ct; pcb[l] = c->lv[l].cbct;
+    }
+    for (int l = nl - 1; l >= 0; --l) {
+        Level& L = c->lv[l];
+        float* r = l == 0 ? out_disp : L.disp;
+        if (l == nl - 1) {
+            if (cudaMemsetAsync(r, 0, 3 * L.N * sizeof(float), st) != cudaSuccess)
+                return fail(c, DISC_ERR_CUDA, "cudaMemsetAsync failed");
+        } else {
+            DISC_TRY(launch_upsample(c, c->lv[l + 1], c->lv[l + 1].disp, r, st));
+        }
+        DISC_TRY(launch_moments<kModeZscore>(c, L, pcb[l], nullptr, L.zhat, nullptr, st));
+        DISC_TRY(launch_warp(c, L, pct[l], r, L.m, st));
+        const bool need_m = (l == 0 && out_corrected_cbct != nullptr);
+        DISC_TRY(iterate_level(c, L, pct[l], r, c->iters, need_m, st));
+        if (need_m)                                                                    // reading A12
+            DISC_TRY(launch_moments<kModeCorrect>(c, L, L.m, L.zhat, out_corrected_cbct, nullptr, st));
+    }
+    return DISC_OK;
+}
+
+disc_status disc_register_host(disc_ctx* c, const float* ct_host, const float* cbct_host, float* out_disp_host,
+                               float* out_corr_host, void* stream) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_NEED(c, ct_host && cbct_host && out_disp_host, "NULL pointer");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t b = c->lv[0].N * sizeof(float);
+    if (!c->h2d_ct) {
+        bool ok = cudaMalloc(&c->h2d_ct, b) == cudaSuccess && cudaMalloc(&c->h2d_cbct, b) == cudaSuccess &&
+                  cudaMalloc(&c->d_out_disp, 3 * b) == cudaSuccess && cudaMalloc(&c->d_out_corr, b) == cudaSuccess;
+        if (!ok) { cudaGetLastError(); return fail(c, DISC_ERR_ALLOC, "cudaMalloc (host staging) failed"); }
+    }
+    if (cudaMemcpyAsync(c->h2d_ct, ct_host, b, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(c->h2d_cbct, cbct_host, b, cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return fail(c, DISC_ERR_CUDA, "H2D copy failed: %s", cudaGetErrorString(cudaGetLastError()));
+    DISC_TRY(disc_register(c, c->h2d_ct, c->h2d_cbct, c->d_out_disp, out_corr_host ? c->d_out_corr : nullptr, stream));
+    if (cudaMemcpyAsync(out_disp_host, c->d_out_disp, 3 * b, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+        return fail(c, DISC_ERR_CUDA, "D2H copy failed");
+    if (out_corr_host && cudaMemcpyAsync(out_corr_host, c->d_out_corr, b, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+        return fail(c, DISC_ERR_CUDA, "D2H copy failed");
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail(c, DISC_ERR_CUDA, "stream sync: %s", cudaGetErrorString(e));
+    return DISC_OK;
+}
+
+disc_status disc_box_moments(disc_ctx* c, int level, const float* vol, float* mean, float* var, void* stream) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_NEED(c, level_ok(c, level), "level out of range");
+    DISC_NEED(c, vol && mean && var, "NULL pointer");
+    return launch_moments<kModeMoments>(c, c->lv[level], vol, nullptr, mean, var, (cudaStream_t)stream);
+}
+
+disc_status disc_force_update(disc_ctx* c, int level, const float* m, const float* s, float* disp_inout, void* stream) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_NEED(c, level_ok(c, level), "level out of range");
+    DISC_NEED(c, m && s && disp_inout, "NULL pointer");
+    const Level& L = c->lv[level];
+    launch_force_update(m, s, disp_inout, L.nx, L.ny, L.nz, DISC_EPS_DEN, (cudaStream_t)stream);
+    return check_launch(c, "k_force_update");
+}
+
+disc_status disc_smooth_field(disc_ctx* c, int level, float* disp_inout, void* stream) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_NEED(c, level_ok(c, level), "level out of range");
+    DISC_NEED(c, disp_inout, "NULL pointer");
+    Level& L = c->lv[level];
+    cudaStream_t st = (cudaStream_t)stream;
+    DISC_TRY(launch_force_gxy<false>(c, L, nullptr, nullptr, disp_inout, L.scratch, st));
+    return launch_gz_warp<false>(c, L, L.scratch, disp_inout, nullptr, nullptr, st);
+}
+
+disc_status disc_downsample(disc_ctx* c, int level_from, const float* vol, float* out, void* stream) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_NEED(c, level_from >= 0 && level_from + 1 < c->levels, "level_from out of range");
+    DISC_NEED(c, vol && out, "NULL pointer");
+    return launch_downsample(c, c->lv[level_from], vol, out, (cudaStream_t)stream);
+}
+
+disc_status disc_upsample_field(disc_ctx* c, int level_from, const float* disp, float* out, void* stream) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_NEED(c, level_from >= 1 && level_from < c->levels, "level_from out of range");
+    DISC_NEED(c, disp && out, "NULL pointer");
+    return launch_upsample(c, c->lv[level_from], disp, out, (cudaStream_t)stream);
+}
+
+}  // extern "C"

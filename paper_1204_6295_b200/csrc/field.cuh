@@ -1,0 +1,187 @@
+// field.cuh -- the displacement-field kernels: force + update, Gaussian regularisation, warp.
+//
+// Steps (c) and (d) of an iteration plus the warp (b) that opens the next one:
+//   k_force_gxy<K, FORCE> : [r += force(m, s')]  then the x and y Gaussian passes   -> scratch field
+//   k_gz_warp<K, WARP>    : the z Gaussian pass of the scratch field -> r, [then m = ct(x + r(x))]
+// Fusing the force into the x/y passes and the warp into the z pass removes one read of r (12 B/voxel)
+// and one read + one write of the un-smoothed field per iteration; the stand-alone variants
+// (FORCE = false, WARP = false) serve disc_smooth_field.
+//
+// Force (Eq. 1, first term, with the corrected CBCT s'; readings A1, A2, A7, A8):
+//   g = central difference of s' with clamped indices, d = s' - m, r_c += d g_c / (|g|^2 + d^2 + eps).
+// Gaussian (reading A10): taps w[-K..K], replicate border, passes x, y, z.
+// Both marching passes keep their (2K+1)-deep window in REGISTERS, statically indexed through a loop
+// unrolled 2K+1 times; threads map to x so every global access is a coalesced row segment.
+#pragma once
+#include "common.cuh"
+
+namespace disc {
+
+// r_c(x,y,z) after the force update (or just r_c when FORCE = false); x,y,z must be in range.
+template <bool FORCE>
+__device__ __forceinline__ void updated_field(const float* __restrict__ m, const float* __restrict__ s,
+                                              const float* __restrict__ rin, int nx, int ny, int nz, size_t N,
+                                              int x, int y, int z, float eps_den, float out[3]) {
+    const size_t plane = (size_t)nx * ny;
+    const size_t i = (size_t)z * plane + (size_t)y * nx + x;
+    out[0] = __ldg(rin + i);
+    out[1] = __ldg(rin + N + i);
+    out[2] = __ldg(rin + 2 * N + i);
+    if (FORCE) {
+        const float sc = __ldg(s + i);
+        const float gx = 0.5f * (__ldg(s + i + (x < nx - 1 ? 1 : 0)) - __ldg(s + i - (x > 0 ? 1 : 0)));
+        const float gy = 0.5f * (__ldg(s + i + (y < ny - 1 ? (size_t)nx : 0)) - __ldg(s + i - (y > 0 ? (size_t)nx : 0)));
+        const float gz = 0.5f * (__ldg(s + i + (z < nz - 1 ? plane : 0)) - __ldg(s + i - (z > 0 ? plane : 0)));
+        const float d = sc - __ldg(m + i);
+        const float den = fmaf(gx, gx, fmaf(gy, gy, fmaf(gz, gz, fmaf(d, d, eps_den))));
+        const float q = d / den;
+        out[0] = fmaf(q, gx, out[0]);
+        out[1] = fmaf(q, gy, out[1]);
+        out[2] = fmaf(q, gz, out[2]);
+    }
+}
+
+// Step (c) alone, in place (disc_force_update).
+static __global__ void __launch_bounds__(256)
+k_force_update(const float* __restrict__ m, const float* __restrict__ s, float* __restrict__ r, int nx, int ny,
+               int nz, float eps_den) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y, z = blockIdx.z;
+    if (x >= nx) return;
+    const size_t N = (size_t)nx * ny * nz;
+    float u[3];
+    updated_field<true>(m, s, r, nx, ny, nz, N, x, y, z, eps_den, u);
+    const size_t i = ((size_t)z * ny + y) * nx + x;
+    r[i] = u[0]; r[N + i] = u[1]; r[2 * N + i] = u[2];
+}
+
+// [force + update] + Gaussian x + Gaussian y.  Grid (x tiles, y segments, z); TXB threads <-> x.
+template <int K, bool FORCE, int TXB>
+__global__ void __launch_bounds__(TXB)
+k_force_gxy(const float* __restrict__ m, const float* __restrict__ s, const float* __restrict__ rin,
+            float* __restrict__ rout, int nx, int ny, int nz, int yseg, float eps_den, GaussTaps gw) {
+    constexpr int W = 2 * K + 1;
+    __shared__ float row[2][3][TXB + 2 * K];
+    const int tid = threadIdx.x;
+    const int x0 = blockIdx.x * TXB;
+    const int x = x0 + tid;
+    const int xc = min(x, nx - 1);
+    const int z = blockIdx.z;
+    const int y0 = blockIdx.y * yseg, y1 = min(y0 + yseg, ny);
+    const size_t N = (size_t)nx * ny * nz;
+    const size_t plane = (size_t)nx * ny;
+    // halo duty: threads 0..K-1 take the left halo, K..2K-1 the right halo
+    const bool halo = tid < 2 * K;
+    const int hx = clampi(tid < K ? x0 - K + tid : x0 + TXB + (tid - K), 0, nx - 1);
+    const int hslot = tid < K ? tid : TXB + tid;  // tid>=K: K + TXB + (tid-K)
+
+    float ring[3][W];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int j = 0; j < W; ++j) ring[c][j] = 0.f;
+
+    // rows yy = y0-K .. y1-1+K enter in order; row (yy) lives in ring slot (yy - (y0-K)) % W
+    const int yend = y1 + K;
+    int buf = 0;
+    for (int yb = y0 - K; yb < yend; yb += W) {
+#pragma unroll
+        for (int j = 0; j < W; ++j) {
+            const int yy = yb + j;
+            if (yy >= yend) break;
+            const int yr = clampi(yy, 0, ny - 1);  // replicate border in y
+            float u[3];
+            updated_field<FORCE>(m, s, rin, nx, ny, nz, N, xc, yr, z, eps_den, u);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) row[buf][c][K + tid] = u[c];
+            if (halo) {
+                float h[3];
+                updated_field<FORCE>(m, s, rin, nx, ny, nz, N, hx, yr, z, eps_den, h);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) row[buf][c][hslot] = h[c];
+            }
+            __syncthreads();
+            // x pass: replicate border in x is already in the row (positions were clamped)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                float acc = 0.f;
+#pragma unroll
+                for (int k = 0; k < W; ++k) acc = fmaf(gw.w[k], row[buf][c][tid + k], acc);
+                ring[c][j] = acc;
+            }
+            buf ^= 1;  // the other buffer was last read before the previous barrier
+            // y pass: output row yo = yy - K uses rows yo-K..yo+K = slots (j+1+k) % W, k = 0..2K
+            const int yo = yy - K;
+            if (yo >= y0 && x < nx) {
+                const size_t o = (size_t)z * plane + (size_t)yo * nx + x;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    float acc = 0.f;
+#pragma unroll
+                    for (int k = 0; k < W; ++k) acc = fmaf(gw.w[k], ring[c][(j + 1 + k) % W], acc);
+                    rout[c * N + o] = acc;
+                }
+            }
+        }
+    }
+}
+
+// Gaussian z pass (+ warp of the moving image by the finished field).  Threads <-> (x,y) columns.
+template <int K, bool WARP>
+__global__ void __launch_bounds__(128)
+k_gz_warp(const float* __restrict__ rin, float* __restrict__ rout, const float* __restrict__ moving,
+          float* __restrict__ mout, int nx, int ny, int nz, int zchunk, GaussTaps gw) {
+    constexpr int W = 2 * K + 1;
+    const size_t plane = (size_t)nx * ny;
+    const size_t col = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= plane) return;
+    const size_t N = plane * nz;
+    const int z0 = blockIdx.y * zchunk, z1 = min(z0 + zchunk, nz);
+    const int y = (int)(col / nx), x = (int)(col - (size_t)y * nx);
+
+    float ring[3][W];
+    // slices z0-K .. z0+K-1 into slots 0 .. 2K-1
+#pragma unroll
+    for (int j = 0; j < W - 1; ++j) {
+        const size_t o = (size_t)clampi(z0 - K + j, 0, nz - 1) * plane + col;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) ring[c][j] = __ldg(rin + c * N + o);
+    }
+    for (int zb = z0; zb < z1; zb += W) {
+#pragma unroll
+        for (int j = 0; j < W; ++j) {
+            const int z = zb + j;
+            if (z >= z1) break;
+            const size_t oin = (size_t)clampi(z + K, 0, nz - 1) * plane + col;  // replicate border in z
+#pragma unroll
+            for (int c = 0; c < 3; ++c) ring[c][(j + W - 1) % W] = __ldg(rin + c * N + oin);
+            float r[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                float acc = 0.f;
+#pragma unroll
+                for (int k = 0; k < W; ++k) acc = fmaf(gw.w[k], ring[c][(j + k) % W], acc);
+                r[c] = acc;
+            }
+            const size_t o = (size_t)z * plane + col;
+            rout[o] = r[0]; rout[N + o] = r[1]; rout[2 * N + o] = r[2];
+            if (WARP)
+                mout[o] = trilinear_clamped(moving, nx, ny, nz, (float)x + r[0], (float)y + r[1], (float)z + r[2]);
+        }
+    }
+}
+
+// Step (b) alone (disc_warp).
+static __global__ void __launch_bounds__(256)
+k_warp(const float* __restrict__ moving, const float* __restrict__ r, float* __restrict__ out, int nx, int ny,
+       int nz) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y, z = blockIdx.z;
+    if (x >= nx) return;
+    const size_t N = (size_t)nx * ny * nz;
+    const size_t i = ((size_t)z * ny + y) * nx + x;
+    out[i] = trilinear_clamped(moving, nx, ny, nz, (float)x + __ldg(r + i), (float)y + __ldg(r + N + i),
+                               (float)z + __ldg(r + 2 * N + i));
+}
+
+}  // namespace disc

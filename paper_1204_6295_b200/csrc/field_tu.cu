@@ -1,0 +1,104 @@
+// field_tu.cu -- instantiates k_force_gxy<K,...> and k_gz_warp<K,...> for K in [DISC_K_LO, DISC_K_HI]; built
+// once per range (-DDISC_TU=n -DDISC_K_LO=a -DDISC_K_HI=b).  TU 0 also holds the K-independent kernels.
+#include "field.cuh"
+#include "launch.h"
+
+#define DISC_CAT2(a, b) a##b
+#define DISC_CAT(a, b) DISC_CAT2(a, b)
+
+namespace disc {
+
+template <int K, bool FORCE>
+static void launch_fg(int txb, const float* m, const float* s, const float* rin, float* rout, int nx, int ny, int nz,
+                      int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
+    dim3 grid((nx + txb - 1) / txb, (ny + yseg - 1) / yseg, nz);
+    if (txb == 128)
+        k_force_gxy<K, FORCE, 128><<<grid, 128, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps);
+    else if (txb == 64)
+        k_force_gxy<K, FORCE, 64><<<grid, 64, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps);
+    else
+        k_force_gxy<K, FORCE, 32><<<grid, 32, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps);
+}
+
+template <int K, bool WARP>
+static void launch_gz(const float* rin, float* rout, const float* moving, float* mout, int nx, int ny, int nz,
+                      int zchunk, const GaussTaps& taps, cudaStream_t st) {
+    const size_t plane = (size_t)nx * ny;
+    dim3 grid((unsigned)((plane + 127) / 128), (nz + zchunk - 1) / zchunk, 1);
+    k_gz_warp<K, WARP><<<grid, 128, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps);
+}
+
+#define DISC_IN(k) ((k) >= DISC_K_LO && (k) <= DISC_K_HI)
+#define DISC_KK(k) (DISC_IN(k) ? (k) : DISC_K_LO)
+#define DISC_FOR_K(X) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12)
+
+bool DISC_CAT(launch_force_gxy_tu, DISC_TU)(int K, bool force, int txb, const float* m, const float* s,
+                                            const float* rin, float* rout, int nx, int ny, int nz, int yseg,
+                                            float eps_den, const GaussTaps& taps, cudaStream_t st) {
+    switch (K) {
+#define DISC_CASE(k)                                                                                       \
+    case k:                                                                                                \
+        if (!DISC_IN(k)) return false;                                                                     \
+        if (force) launch_fg<DISC_KK(k), true>(txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);  \
+        else launch_fg<DISC_KK(k), false>(txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);       \
+        return true;
+        DISC_FOR_K(DISC_CASE)
+#undef DISC_CASE
+    }
+    return false;
+}
+
+bool DISC_CAT(launch_gz_warp_tu, DISC_TU)(int K, bool warp, const float* rin, float* rout, const float* moving,
+                                          float* mout, int nx, int ny, int nz, int zchunk, const GaussTaps& taps,
+                                          cudaStream_t st) {
+    switch (K) {
+#define DISC_CASE(k)                                                                                 \
+    case k:                                                                                          \
+        if (!DISC_IN(k)) return false;                                                               \
+        if (warp) launch_gz<DISC_KK(k), true>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st); \
+        else launch_gz<DISC_KK(k), false>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st);     \
+        return true;
+        DISC_FOR_K(DISC_CASE)
+#undef DISC_CASE
+    }
+    return false;
+}
+
+#if DISC_TU == 0
+void launch_force_update(const float* m, const float* s, float* r, int nx, int ny, int nz, float eps_den,
+                         cudaStream_t st) {
+    dim3 grid((nx + 255) / 256, ny, nz);
+    k_force_update<<<grid, 256, 0, st>>>(m, s, r, nx, ny, nz, eps_den);
+}
+
+void launch_warp_kernel(const float* moving, const float* r, float* out, int nx, int ny, int nz, cudaStream_t st) {
+    dim3 grid((nx + 255) / 256, ny, nz);
+    k_warp<<<grid, 256, 0, st>>>(moving, r, out, nx, ny, nz);
+}
+
+bool launch_moments_any(int R, int mode, const float* vol, const float* aux, float* out0, float* out1, int nx,
+                        int ny, int nz, int zchunk, float eps_var, cudaStream_t st) {
+    return launch_moments_tu0(R, mode, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st) ||
+           launch_moments_tu1(R, mode, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st) ||
+           launch_moments_tu2(R, mode, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st) ||
+           launch_moments_tu3(R, mode, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st);
+}
+
+bool launch_force_gxy_any(int K, bool force, int txb, const float* m, const float* s, const float* rin, float* rout,
+                          int nx, int ny, int nz, int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
+    return launch_force_gxy_tu0(K, force, txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st) ||
+           launch_force_gxy_tu1(K, force, txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st) ||
+           launch_force_gxy_tu2(K, force, txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st) ||
+           launch_force_gxy_tu3(K, force, txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
+}
+
+bool launch_gz_warp_any(int K, bool warp, const float* rin, float* rout, const float* moving, float* mout, int nx,
+                        int ny, int nz, int zchunk, const GaussTaps& taps, cudaStream_t st) {
+    return launch_gz_warp_tu0(K, warp, rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st) ||
+           launch_gz_warp_tu1(K, warp, rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st) ||
+           launch_gz_warp_tu2(K, warp, rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st) ||
+           launch_gz_warp_tu3(K, warp, rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st);
+}
+#endif
+
+}  // namespace disc

@@ -1,0 +1,104 @@
+"""Whole-schedule parity: disc_register / disc_iterate on the GPU against oracle.register on the same seeded
+phantoms.  Tolerance (north_star): final displacement max-abs <= 1e-2 voxel after the full schedule; corrected
+CBCT max-abs <= 1e-4 x intensity range (plus the field tolerance times the steepest edge, because the corrected
+image is evaluated at the GPU's own final field)."""
+import numpy as np
+import pytest
+
+import phantoms
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def disc():
+    import __graft_entry__
+    __graft_entry__.build()
+    import paper_1204_6295_b200 as d
+    assert torch.cuda.is_available()
+    return d
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def gpu_register(disc, ct, cbct, R, sigma, levels, iters, host=False):
+    nz, ny, nx = ct.shape
+    ctx = disc.disc_create((nx, ny, nz), (1.0, 1.0, 1.0), R, sigma, levels, iters)
+    if host:
+        r = np.empty((3,) + ct.shape, dtype=np.float32)
+        corr = np.empty_like(ct)
+        disc.disc_register_host(ctx, ct, cbct, r, corr)
+    else:
+        d_r = torch.empty((3,) + ct.shape, device="cuda")
+        d_c = torch.empty(ct.shape, device="cuda")
+        disc.disc_register(ctx, dev(ct), dev(cbct), d_r, d_c)
+        torch.cuda.synchronize()
+        r, corr = d_r.cpu().numpy(), d_c.cpu().numpy()
+    n = disc.disc_launch_count(ctx)
+    disc.disc_destroy(ctx)
+    return r, corr, n
+
+
+def check(ct, cbct, r, corr, r_ref, corr_ref):
+    err_r = np.abs(r - r_ref).max()
+    assert err_r <= 1e-2, f"field error {err_r} voxel"
+    rng = float(max(ct.max(), cbct.max()) - min(ct.min(), cbct.min()))
+    g = np.abs(np.stack(np.gradient(ct.astype(np.float64)))).max()
+    err_c = np.abs(corr - corr_ref).max()
+    assert err_c <= 1e-4 * rng + 2.0 * err_r * g + 1e-3, f"corrected cbct error {err_c} HU (field err {err_r}, grad {g})"
+    return err_r, err_c
+
+
+@pytest.mark.parametrize("dims,R,sigma,levels,iters", [
+    ((24, 20, 12), 1, 1.0, 1, 5),
+    ((40, 36, 20), 2, 1.5, 2, 10),
+    ((70, 44, 24), 3, 2.0, 3, 8),        # ragged tiles at every level
+    ((32, 32, 16), 0, 1.5, 1, 4),        # R = 0: s' = m, no force
+])
+def test_register_small(disc, oracle_mod, dims, R, sigma, levels, iters):
+    dims = tuple(d - d % (1 << (levels - 1)) for d in dims)
+    ct, cbct, _, _ = phantoms.make_pair(1, dims=dims)
+    r, corr, n = gpu_register(disc, ct, cbct, R, sigma, levels, iters)
+    r_ref, corr_ref = oracle_mod.register(ct, cbct, R, sigma, levels, iters)
+    check(ct, cbct, r, corr, r_ref, corr_ref)
+    assert n >= 3 * levels * iters
+
+
+def test_register_config1_full_schedule(disc, oracle_mod):
+    ct, cbct, u, p = phantoms.make_pair(1)
+    args = (p["patch_radius"], p["sigma"], p["levels"], p["iters"])
+    r, corr, _ = gpu_register(disc, ct, cbct, *args)
+    r_ref, corr_ref = oracle_mod.register(ct, cbct, *args)
+    err_r, err_c = check(ct, cbct, r, corr, r_ref, corr_ref)
+    print(f"config 1: max|dr| = {err_r:.2e} voxel, max|dcorr| = {err_c:.2e} HU")
+    # the host-buffer entry point gives the same answer
+    r2, corr2, _ = gpu_register(disc, ct, cbct, *args, host=True)
+    assert np.array_equal(r2, r) and np.array_equal(corr2, corr)
+
+
+@pytest.mark.slow
+def test_register_config2_full_schedule(disc, oracle_mod):
+    ct, cbct, u, p = phantoms.make_pair(2)
+    args = (p["patch_radius"], p["sigma"], p["levels"], p["iters"])
+    r, corr, _ = gpu_register(disc, ct, cbct, *args)
+    r_ref, corr_ref = oracle_mod.register(ct, cbct, *args)
+    err_r, err_c = check(ct, cbct, r, corr, r_ref, corr_ref)
+    print(f"config 2: max|dr| = {err_r:.2e} voxel, max|dcorr| = {err_c:.2e} HU")
+
+
+def test_iterate_matches_stepwise_oracle(disc, oracle_mod):
+    ct, cbct, _, _ = phantoms.make_pair(1, dims=(48, 40, 24))
+    R, sigma, n_it = 2, 1.5, 6
+    r0 = (0.5 * phantoms.disp_smooth_random((48, 40, 24), np.random.default_rng(3), max_disp=2.0)).astype(np.float32)
+    ctx = disc.disc_create((48, 40, 24), (1, 1, 1), R, sigma, 1, n_it)
+    d_r = dev(r0)
+    disc.disc_iterate(ctx, 0, dev(ct), dev(cbct), d_r, n_it)
+    rr = r0.copy()
+    for _ in range(n_it):
+        m = oracle_mod.warp(ct, rr)
+        rr = oracle_mod.demons_step(m, oracle_mod.correct(cbct, m, R), rr, sigma)
+    assert np.abs(d_r.cpu().numpy() - rr).max() <= 1e-3
