@@ -1,0 +1,298 @@
+#!/usr/bin/env python
+"""bench.py -- measures the DISC hot path on B200 (and, with --impl reference, the CPU oracle).
+
+Workload (BASELINE.json configs[2], the one `metric` is quoted on): 256x256x128 fp32 head-and-neck phantom,
+3-level pyramid, 100 iterations per level, patch 11^3 (R = 5), Gaussian sigma 2.0.  Synthetic, seeded.
+
+One "step" = one whole registration (`disc_register`): both pyramids, 3 x 100 iterations of
+{warp, moments+correct, force+update, Gaussian}, two field up-samplings, final corrected CBCT.
+`value` = voxel-updates/s over the whole schedule (sum over levels of N_level x iterations, / time), inputs
+resident in HBM; `iterations_per_s_finest` = steady-state iterations/s on the 256x256x128 level alone;
+`e2e` = the same metric through `disc_register_host` with pinned HOST buffers (H2D + D2H inside the timing).
+
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for the roofline arithmetic.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+WORKLOAD_CONFIG = 3
+# algorithmic (compulsory) bytes per voxel of the three per-iteration kernels -- DESIGN.md "Kernels"
+KERNELS = (
+    ("moments_correct", 12.0),   # read m 4 + cached CBCT z-score 4, write s' 4
+    ("force_gauss_xy", 32.0),    # read m 4 + s' 4 + r 12, write r~ 12
+    ("gauss_z_warp", 32.0),      # read r~ 12, write r 12, gather ct 4, write m 4
+)
+
+
+def schedule_voxel_updates(dims, levels, iters):
+    nx, ny, nz = dims
+    return sum((nx >> l) * (ny >> l) * (nz >> l) * iters for l in range(levels))
+
+
+def measured_peak_gbs():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs"""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.p = index, None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if not self.p:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+            out, _ = self.p.communicate()
+        sm, mx, reasons = [], [], set()
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 8:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[4:8]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        busy = [v for v in sm if v > 0.5 * max(mx or [1])] or sm
+        return {"sm_mhz": statistics.median(busy) if busy else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(ct, cbct, R, sigma, n_iter):
+    """n_iter finest-level iterations of the oracle as it stands (stepwise functions), timed on the host cores."""
+    import numpy as np
+    import oracle
+    r = np.zeros((3,) + ct.shape, dtype=np.float32)
+    mu_s, var_s = oracle.box_moments(cbct, R)     # once per level in the schedule (1/100 of it): outside the timing
+    t0 = time.perf_counter()
+    for _ in range(n_iter):
+        m = oracle.warp(ct, r)
+        mu_m, var_m = oracle.box_moments(m, R)
+        sp = oracle.correct_from_moments(cbct, mu_s, var_s, mu_m, var_m)
+        r = oracle.demons_step(m, sp, r, sigma)
+    dt = time.perf_counter() - t0
+    return ct.size * n_iter / dt, dt, oracle.num_threads()
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the same config/metric, each step a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import phantoms
+    ct, cbct, _, p = phantoms.make_pair(WORKLOAD_CONFIG)
+    R, sigma = p["patch_radius"], p["sigma"]
+    sample = "1 finest-level iteration (256x256x128, R=5, sigma=2) of the config-3 schedule per step"
+    for _ in range(args.warmup):
+        oracle_sample(ct, cbct, R, sigma, 1)
+    t0 = time.perf_counter()
+    cores = 1
+    for _ in range(args.steps):
+        _, _, cores = oracle_sample(ct, cbct, R, sigma, 1)
+    dt = time.perf_counter() - t0
+    value = ct.size * args.steps / dt
+    line = {
+        "impl": "reference", "metric": "voxel_updates_per_sec", "value": value, "unit": "voxel-updates/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config3 256x256x128 R=5 sigma=2.0 (oracle sample)", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "voxel-updates/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "voxel-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="disc", choices=["disc", "reference"])
+    ap.add_argument("--config", type=int, default=WORKLOAD_CONFIG, help="BASELINE.json config (bench line: 3)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+
+    import paper_1204_6295_b200 as disc
+    import phantoms
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    # replicas only: every rank registers its own seeded pair; no data-path collective
+    ct, cbct, _, p = phantoms.make_pair(args.config)
+    nz, ny, nx = ct.shape
+    dims = (nx, ny, nz)
+    R, sigma, levels, iters = p["patch_radius"], p["sigma"], p["levels"], p["iters"]
+    ctx = disc.disc_create(dims, (1.0, 1.0, 1.0), R, sigma, levels, iters)
+    d_ct, d_cb = torch.from_numpy(ct).cuda(), torch.from_numpy(cbct).cuda()
+    d_r = torch.empty((3, nz, ny, nx), device="cuda")
+    d_corr = torch.empty((nz, ny, nx), device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(ms):
+        if dist is None:
+            return ms
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ---------------- device-resident: K whole registrations
+    for _ in range(args.warmup):
+        disc.disc_register(ctx, d_ct, d_cb, d_r, d_corr)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = disc.disc_launch_count(ctx)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        disc.disc_register(ctx, d_ct, d_cb, d_r, d_corr)
+    e1.record(stream)
+    barrier()
+    ms_total = max_over_ranks(e0.elapsed_time(e1))
+    launches = disc.disc_launch_count(ctx) - l0
+    vu_step = schedule_voxel_updates(dims, levels, iters)
+    value = world * vu_step * args.steps / (ms_total * 1e-3)
+
+    # ---------------- steady-state finest level + per-kernel durations (CUDA events inside the library)
+    n_prof = 50
+    d_r2 = d_r.clone()
+    disc.disc_profile_iteration(ctx, 0, d_ct, d_cb, d_r2, 5)                 # warm-up
+    kms = disc.disc_profile_iteration(ctx, 0, d_ct, d_cb, d_r2, n_prof)
+    d_r2.copy_(d_r)
+    disc.disc_iterate(ctx, 0, d_ct, d_cb, d_r2, 5)
+    torch.cuda.synchronize()
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f0.record(stream)
+    disc.disc_iterate(ctx, 0, d_ct, d_cb, d_r2, 100)
+    f1.record(stream)
+    torch.cuda.synchronize()
+    ms_iter = f0.elapsed_time(f1) / 100.0          # includes the per-call z-score + warp prologue (2 of 302 launches)
+    clocks = sampler.stop() if rank == 0 else None
+
+    # ---------------- end to end: pinned host buffers through disc_register_host
+    h_ct, h_cb = torch.from_numpy(ct).pin_memory(), torch.from_numpy(cbct).pin_memory()
+    h_r = torch.empty((3, nz, ny, nx), dtype=torch.float32).pin_memory()
+    h_corr = torch.empty((nz, ny, nx), dtype=torch.float32).pin_memory()
+    disc.disc_register_host(ctx, h_ct, h_cb, h_r, h_corr)
+    barrier()
+    t0 = time.perf_counter()
+    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    g0.record(stream)
+    n_e2e = max(1, min(args.steps, 3))
+    for _ in range(n_e2e):
+        disc.disc_register_host(ctx, h_ct, h_cb, h_r, h_corr)
+    g1.record(stream)
+    barrier()
+    ms_e2e = max_over_ranks(g0.elapsed_time(g1))
+    e2e_value = world * vu_step * n_e2e / (ms_e2e * 1e-3)
+    n0 = nx * ny * nz
+    h2d, d2h = 2 * 4 * n0, 4 * 4 * n0
+
+    if rank != 0:
+        disc.disc_destroy(ctx)
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # ---------------- roofline of the dominant kernel
+    peak, peak_src = measured_peak_gbs()
+    per_kernel = []
+    for (name, bpv), ms in zip(KERNELS, kms):
+        gbs = bpv * n0 / (ms * 1e-3) / 1e9
+        per_kernel.append({"kernel": name, "ms": ms, "bytes_per_voxel": bpv, "gbs": gbs, "frac": gbs / peak})
+    dom = max(per_kernel, key=lambda k: k["ms"])
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")     # written from an `ncu --set full` capture, per launch
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(dom["kernel"])
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["gbs"], "peak": peak, "unit": "GB/s",
+                "frac": dom["gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": dom["bytes_per_voxel"] * n0, "per_kernel": per_kernel,
+                "iteration_gbs": 76.0 * n0 / (ms_iter * 1e-3) / 1e9, "iteration_frac": 76.0 * n0 / (ms_iter * 1e-3) / 1e9 / peak}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        v, dt, cores = oracle_sample(ct, cbct, R, sigma, 3)
+        cpu = {"value": v, "unit": "voxel-updates/s", "cores": cores, "kind": "oracle",
+               "sample": f"3 finest-level iterations (256x256x128, R={R}, sigma={sigma}) of the config-3 schedule, {dt:.1f} s"}
+
+    line = {
+        "metric": "voxel_updates_per_sec", "value": value, "unit": "voxel-updates/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32 (patch sums f64)", "data": "synthetic",
+        "config": {"workload": f"config{args.config} {nx}x{ny}x{nz} phantom, {levels}-level pyramid, {iters} iters/level, "
+                               f"patch {2 * R + 1}^3, sigma {sigma}", "multi_gpu": "replicas only",
+                   "l2": "working set 320 MiB > 126 MB L2 (inputs larger than L2)"},
+        "iterations_per_s_finest": 1e3 / ms_iter, "voxel_updates_per_s_finest": n0 * 1e3 / ms_iter,
+        "ms_per_iteration_finest": ms_iter,
+        "e2e": {"value": e2e_value, "unit": "voxel-updates/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": ms_e2e / n_e2e},
+        "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+    disc.disc_destroy(ctx)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -118,6 +118,13 @@ disc_status disc_register_host(disc_ctx* ctx, const float* ct_host, const float*
 disc_status disc_iterate(disc_ctx* ctx, int level, const float* ct, const float* cbct, float* disp_inout,
                          int n_iters, void* stream);
 
+/* Measurement aid for bench.py's roofline object: runs `n_iters` iterations exactly as disc_iterate does, with a
+ * CUDA event pair around every kernel on `stream`, SYNCHRONISES the stream and writes the mean duration in
+ * milliseconds of each of the three per-iteration kernels to ms_per_kernel (HOST, 3 floats):
+ * [0] moments+correct, [1] force+update+Gaussian x,y, [2] Gaussian z + warp. */
+disc_status disc_profile_iteration(disc_ctx* ctx, int level, const float* ct, const float* cbct, float* disp_inout,
+                                   int n_iters, float ms_per_kernel[3], void* stream);
+
 /* ---- finer-grained exports (BASELINE.json config 5 per-kernel sweep, and tests) ---- */
 
 /* Patch mean and population variance of `vol` over the truncated cube of radius R (Eq. 3, A4).

@@ -104,6 +104,17 @@ def correct(cbct, ct_warped, R, eps_var=EPS_VAR):
     return out
 
 
+def correct_from_moments(cbct, mu_s, var_s, mu_m, var_m, eps_var=EPS_VAR):
+    """Eqs. (5)-(6) applied with given patch moments (the driver computes the CBCT's once per level)."""
+    L = _load()
+    s, ps = _f32(cbct)
+    arrs = [np.ascontiguousarray(a, dtype=np.float64) for a in (mu_s, var_s, mu_m, var_m)]
+    out = np.empty_like(s)
+    L.oracle_correct_from_moments(ps, *[a.ctypes.data_as(_f64p) for a in arrs], ctypes.c_size_t(s.size),
+                                  ctypes.c_double(eps_var), out.ctypes.data_as(_f32p))
+    return out
+
+
 def correct_at(cbct, ct_warped, R, idx, eps_var=EPS_VAR):
     L = _load()
     s, ps = _f32(cbct)

@@ -24,7 +24,7 @@ DISC_EPS_DEN = 1e-3
 EXPORTS = (
     "disc_create", "disc_destroy", "disc_last_error", "disc_launch_count", "disc_warp", "disc_correct_intensity",
     "disc_demons_step", "disc_register", "disc_register_host", "disc_iterate", "disc_box_moments",
-    "disc_force_update", "disc_smooth_field", "disc_downsample", "disc_upsample_field",
+    "disc_force_update", "disc_smooth_field", "disc_downsample", "disc_upsample_field", "disc_profile_iteration",
 )
 
 if not os.path.exists(LIB_PATH):
@@ -55,6 +55,8 @@ _lib.disc_register_host.restype = _i
 _lib.disc_register_host.argtypes = [_vp] * 6
 _lib.disc_iterate.restype = _i
 _lib.disc_iterate.argtypes = [_vp, _i, _vp, _vp, _vp, _i, _vp]
+_lib.disc_profile_iteration.restype = _i
+_lib.disc_profile_iteration.argtypes = [_vp, _i, _vp, _vp, _vp, _i, ctypes.POINTER(ctypes.c_float), _vp]
 
 
 class DiscError(RuntimeError):
@@ -182,6 +184,15 @@ def disc_iterate(ctx, level, ct, cbct, disp_inout, n_iters, stream=None):
     n = ctx.n(level)
     _check(ctx.handle, _lib.disc_iterate(ctx.handle, level, _dev(ct, n), _dev(cbct, n), _dev(disp_inout, _x3(n)),
                                          int(n_iters), _stream(stream)))
+
+
+def disc_profile_iteration(ctx, level, ct, cbct, disp_inout, n_iters, stream=None):
+    """returns the three mean kernel durations in ms (host floats written by the C call)"""
+    n = ctx.n(level)
+    ms = (ctypes.c_float * 3)()
+    _check(ctx.handle, _lib.disc_profile_iteration(ctx.handle, level, _dev(ct, n), _dev(cbct, n),
+                                                   _dev(disp_inout, _x3(n)), int(n_iters), ms, _stream(stream)))
+    return [float(v) for v in ms]
 
 
 def disc_box_moments(ctx, level, vol, mean, var, stream=None):

@@ -286,6 +286,46 @@ disc_status disc_iterate(disc_ctx* c, int level, const float* ct, const float* c
     return iterate_level(c, L, ct, disp_inout, n_iters, true, st);
 }
 
+disc_status disc_profile_iteration(disc_ctx* c, int level, const float* ct, const float* cbct, float* disp_inout,
+                                   int n_iters, float ms_per_kernel[3], void* stream) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_NEED(c, level_ok(c, level), "level out of range");
+    DISC_NEED(c, ct && cbct && disp_inout && ms_per_kernel, "NULL pointer");
+    DISC_NEED(c, n_iters >= 1 && n_iters <= 4096, "n_iters must be in 1..4096");
+    Level& L = c->lv[level];
+    cudaStream_t st = (cudaStream_t)stream;
+    const int ne = 4 * n_iters;
+    cudaEvent_t* ev = new (std::nothrow) cudaEvent_t[ne];
+    if (!ev) return fail(c, DISC_ERR_ALLOC, "out of host memory");
+    for (int i = 0; i < ne; ++i) cudaEventCreate(&ev[i]);
+    disc_status rc = launch_moments<kModeZscore>(c, L, cbct, nullptr, L.zhat, nullptr, st);
+    if (rc == DISC_OK) rc = launch_warp(c, L, ct, disp_inout, L.m, st);
+    for (int k = 0; k < n_iters && rc == DISC_OK; ++k) {
+        cudaEventRecord(ev[4 * k + 0], st);
+        rc = launch_moments<kModeCorrect>(c, L, L.m, L.zhat, L.sp, nullptr, st);
+        cudaEventRecord(ev[4 * k + 1], st);
+        if (rc == DISC_OK) rc = launch_force_gxy<true>(c, L, L.m, L.sp, disp_inout, L.scratch, st);
+        cudaEventRecord(ev[4 * k + 2], st);
+        if (rc == DISC_OK) rc = launch_gz_warp<true>(c, L, L.scratch, disp_inout, ct, L.m, st);
+        cudaEventRecord(ev[4 * k + 3], st);
+    }
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (rc == DISC_OK && e != cudaSuccess) rc = fail(c, DISC_ERR_CUDA, "stream sync: %s", cudaGetErrorString(e));
+    if (rc == DISC_OK) {
+        double acc[3] = {0, 0, 0};
+        for (int k = 0; k < n_iters; ++k)
+            for (int j = 0; j < 3; ++j) {
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, ev[4 * k + j], ev[4 * k + j + 1]);
+                acc[j] += ms;
+            }
+        for (int j = 0; j < 3; ++j) ms_per_kernel[j] = (float)(acc[j] / n_iters);
+    }
+    for (int i = 0; i < ne; ++i) cudaEventDestroy(ev[i]);
+    delete[] ev;
+    return rc;
+}
+
 disc_status disc_register(disc_ctx* c, const float* ct, const float* cbct, float* out_disp,
                           float* out_corrected_cbct, void* stream) {
     if (!c) return DISC_ERR_INVALID_ARG;
