@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -76,6 +77,12 @@ disc_status check_launch(disc_ctx* c, const char* what) {
         if (!(cond)) return fail((c), DISC_ERR_INVALID_ARG, "%s", (msg));   \
     } while (0)
 
+// optional launch-shape overrides for tuning sweeps (unset in normal use)
+int tune(const char* name, int dflt) {
+    const char* v = std::getenv(name);
+    return v && *v ? std::atoi(v) : dflt;
+}
+
 bool level_ok(const disc_ctx* c, int level) { return level >= 0 && level < c->levels; }
 
 int pick_chunk(int n, int min_chunk, long long ctas_per_chunk, long long target_ctas) {
@@ -95,7 +102,7 @@ disc_status launch_moments(disc_ctx* c, const Level& L, const float* vol, const 
                            float* out1, cudaStream_t st) {
     const int tiles = ((L.nx + kMomTX - 1) / kMomTX) * ((L.ny + kMomTY - 1) / kMomTY);
     const int W = 2 * c->R + 1;
-    const int zchunk = pick_chunk(L.nz, 4 * W > 32 ? 4 * W : 32, tiles, 2 * 148);
+    const int zchunk = tune("DISC_TUNE_MOM_ZCHUNK", pick_chunk(L.nz, 4 * W > 32 ? 4 * W : 32, tiles, 2 * 148));
     if (!launch_moments_any(c->R, MODE, vol, aux, out0, out1, L.nx, L.ny, L.nz, zchunk, DISC_EPS_VAR, st))
         return fail(c, DISC_ERR_UNSUPPORTED, "patch_radius %d > %d", c->R, DISC_MAX_PATCH_RADIUS);
     return check_launch(c, "k_moments");
@@ -107,7 +114,7 @@ disc_status launch_force_gxy(disc_ctx* c, const Level& L, const float* m, const 
     const int txb = L.nx > 64 ? 128 : (L.nx > 32 ? 64 : 32);
     const int xt = (L.nx + txb - 1) / txb;
     const int K = c->K;
-    const int yseg = pick_chunk(L.ny, 8 * K > 32 ? 8 * K : 32, (long long)xt * L.nz, 4 * 148);
+    const int yseg = tune("DISC_TUNE_FG_YSEG", pick_chunk(L.ny, 8 * K > 32 ? 8 * K : 32, (long long)xt * L.nz, 4 * 148));
     if (!launch_force_gxy_any(K, FORCE, txb, m, s, rin, rout, L.nx, L.ny, L.nz, yseg, DISC_EPS_DEN, c->taps, st))
         return fail(c, DISC_ERR_UNSUPPORTED, "Gaussian radius %d unsupported", K);
     return check_launch(c, "k_force_gxy");
@@ -119,7 +126,7 @@ disc_status launch_gz_warp(disc_ctx* c, const Level& L, const float* rin, float*
     const size_t plane = (size_t)L.nx * L.ny;
     const int bx = (int)((plane + 127) / 128);
     const int K = c->K;
-    const int zchunk = pick_chunk(L.nz, 8 * K > 32 ? 8 * K : 32, bx, 8 * 148);
+    const int zchunk = tune("DISC_TUNE_GZ_ZCHUNK", pick_chunk(L.nz, 8 * K > 32 ? 8 * K : 32, bx, 8 * 148));
     if (!launch_gz_warp_any(K, WARP, rin, rout, moving, mout, L.nx, L.ny, L.nz, zchunk, c->taps, st))
         return fail(c, DISC_ERR_UNSUPPORTED, "Gaussian radius %d unsupported", K);
     return check_launch(c, "k_gz_warp");

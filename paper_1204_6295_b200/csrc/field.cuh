@@ -34,7 +34,7 @@ __device__ __forceinline__ void updated_field(const float* __restrict__ m, const
         const float gz = 0.5f * (__ldg(s + i + (z < nz - 1 ? plane : 0)) - __ldg(s + i - (z > 0 ? plane : 0)));
         const float d = sc - __ldg(m + i);
         const float den = fmaf(gx, gx, fmaf(gy, gy, fmaf(gz, gz, fmaf(d, d, eps_den))));
-        const float q = d / den;
+        const float q = __fdividef(d, den);
         out[0] = fmaf(q, gx, out[0]);
         out[1] = fmaf(q, gy, out[1]);
         out[2] = fmaf(q, gz, out[2]);

@@ -1,6 +1,7 @@
 // field_tu.cu -- instantiates k_force_gxy<K,...> and k_gz_warp<K,...> for K in [DISC_K_LO, DISC_K_HI]; built
 // once per range (-DDISC_TU=n -DDISC_K_LO=a -DDISC_K_HI=b).  TU 0 also holds the K-independent kernels.
 #include "field.cuh"
+#include "field_tma.cuh"
 #include "launch.h"
 
 #define DISC_CAT2(a, b) a##b
@@ -8,9 +9,31 @@
 
 namespace disc {
 
+static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+template <int K, bool FORCE, int NT>
+static void launch_fg_tma(const float* m, const float* s, const float* rin, float* rout, int nx, int ny, int nz,
+                          int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
+    using C = FgCfg<K, FORCE, NT>;
+    static bool configured = false;  // one attribute call per instance (idempotent, so a race is harmless)
+    if (!configured) {
+        cudaFuncSetAttribute(k_force_gxy_tma<K, FORCE, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
+        configured = true;
+    }
+    dim3 grid((nx + C::TX - 1) / C::TX, (ny + yseg - 1) / yseg, nz);
+    k_force_gxy_tma<K, FORCE, NT><<<grid, NT, C::smem_bytes, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps);
+}
+
 template <int K, bool FORCE>
 static void launch_fg(int txb, const float* m, const float* s, const float* rin, float* rout, int nx, int ny, int nz,
                       int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
+    const bool tma_ok = nx % 4 == 0 && aligned16(rin) && aligned16(rout) && (!FORCE || (aligned16(m) && aligned16(s)));
+    if (tma_ok) {
+        if (nx > 128) launch_fg_tma<K, FORCE, 128>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
+        else if (nx > 64) launch_fg_tma<K, FORCE, 64>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
+        else launch_fg_tma<K, FORCE, 32>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
+        return;
+    }
     dim3 grid((nx + txb - 1) / txb, (ny + yseg - 1) / yseg, nz);
     if (txb == 128)
         k_force_gxy<K, FORCE, 128><<<grid, 128, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps);
@@ -24,6 +47,11 @@ template <int K, bool WARP>
 static void launch_gz(const float* rin, float* rout, const float* moving, float* mout, int nx, int ny, int nz,
                       int zchunk, const GaussTaps& taps, cudaStream_t st) {
     const size_t plane = (size_t)nx * ny;
+    if (nx % 4 == 0 && aligned16(rin) && aligned16(rout) && (!WARP || aligned16(mout))) {
+        dim3 grid((unsigned)((plane + kGzCols - 1) / kGzCols), (nz + zchunk - 1) / zchunk, 1);
+        k_gz_warp_tma<K, WARP><<<grid, 128, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps);
+        return;
+    }
     dim3 grid((unsigned)((plane + 127) / 128), (nz + zchunk - 1) / zchunk, 1);
     k_gz_warp<K, WARP><<<grid, 128, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps);
 }

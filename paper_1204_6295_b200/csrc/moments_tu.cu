@@ -8,9 +8,62 @@
 
 namespace disc {
 
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point: no link-time dependency on libcuda
+static EncodeTiledFn encode_tiled() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+template <int R>
+static bool launch_r_tma(int mode, const float* vol, const float* aux, float* out0, float* out1, int nx, int ny,
+                         int nz, int zchunk, float eps_var, cudaStream_t st) {
+    using C = MomTmaCfg<R>;
+    EncodeTiledFn enc = encode_tiled();
+    if (!enc) return false;
+    CUtensorMap tmap;
+    const cuuint64_t gdim[3] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz};
+    const cuuint64_t gstr[2] = {(cuuint64_t)nx * 4, (cuuint64_t)nx * ny * 4};
+    const cuuint32_t box[3] = {(cuuint32_t)C::PXB, (cuuint32_t)C::PY, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(vol), gdim, gstr, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return false;
+    static bool configured[3] = {false, false, false};
+    dim3 grid((nx + kMomTX - 1) / kMomTX, (ny + kMomTY - 1) / kMomTY, (nz + zchunk - 1) / zchunk);
+#define DISC_LAUNCH_MODE(M)                                                                                         \
+    {                                                                                                               \
+        if (!configured[M]) {                                                                                       \
+            cudaFuncSetAttribute(k_moments_tma<R, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes); \
+            configured[M] = true;                                                                                   \
+        }                                                                                                           \
+        k_moments_tma<R, M><<<grid, C::NT, C::smem_bytes, st>>>(tmap, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var); \
+    }
+    if (mode == kModeMoments) DISC_LAUNCH_MODE(kModeMoments)
+    else if (mode == kModeZscore) DISC_LAUNCH_MODE(kModeZscore)
+    else DISC_LAUNCH_MODE(kModeCorrect)
+#undef DISC_LAUNCH_MODE
+    return true;
+}
+
 template <int R>
 static void launch_r(int mode, const float* vol, const float* aux, float* out0, float* out1, int nx, int ny, int nz,
                      int zchunk, float eps_var, cudaStream_t st) {
+    // TMA path: rows must be 16-byte multiples and the base 16-byte aligned (tensor-map requirements)
+    if (nx % 4 == 0 && (reinterpret_cast<uintptr_t>(vol) & 15u) == 0 &&
+        launch_r_tma<R>(mode, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st))
+        return;
     dim3 grid((nx + kMomTX - 1) / kMomTX, (ny + kMomTY - 1) / kMomTY, (nz + zchunk - 1) / zchunk);
     constexpr int NT = MomCfg<R>::NT;
     if (mode == kModeMoments)

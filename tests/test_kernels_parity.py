@@ -43,7 +43,9 @@ def rand_pair(shape, seed, noise=20.0):
     return a, b
 
 
-SHAPES = [(7, 6, 5), (9, 17, 33), (20, 45, 70), (32, 64, 64), (1, 1, 9), (3, 40, 2)]
+# nx % 4 == 0 takes the TMA-fed kernels, anything else the plain-load ones; both with ragged tiles
+SHAPES = [(7, 6, 5), (9, 17, 33), (20, 45, 70), (32, 64, 64), (1, 1, 9), (3, 40, 2), (20, 45, 72), (21, 37, 132),
+          (5, 3, 4), (30, 70, 260)]
 
 
 # ------------------------------------------------------------------ warp
@@ -66,7 +68,8 @@ def test_warp(disc, oracle_mod, shape):
 
 # ------------------------------------------------------------------ moments
 @pytest.mark.parametrize("R", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10])
-@pytest.mark.parametrize("shape", [(7, 6, 5), (20, 45, 70), (37, 18, 33)])
+@pytest.mark.parametrize("shape", [(7, 6, 5), (20, 45, 70), (37, 18, 33), (20, 45, 72), (37, 18, 36), (3, 5, 8),
+                                   (26, 50, 100)])
 def test_box_moments(disc, oracle_mod, shape, R):
     vol, _ = rand_pair(shape, 20 + R)
     ctx = make_ctx(disc, shape, R=R)
@@ -81,7 +84,7 @@ def test_box_moments(disc, oracle_mod, shape, R):
 
 def test_box_moments_constant_volume_has_zero_variance(disc):
     """the H1 hazard: E(x^2) - mu^2 must not leak rounding into var (fp32 sums give ~9 HU^2 here)"""
-    shape = (24, 40, 70)
+    shape = (24, 40, 72)
     vol = np.full(shape, 1234.567, dtype=np.float32)
     ctx = make_ctx(disc, shape, R=3)
     mean = torch.empty(shape, device="cuda"); var = torch.empty(shape, device="cuda")
@@ -92,7 +95,7 @@ def test_box_moments_constant_volume_has_zero_variance(disc):
 
 # ------------------------------------------------------------------ correction
 @pytest.mark.parametrize("R", [0, 1, 3, 5, 7, 10])
-@pytest.mark.parametrize("shape", [(7, 6, 5), (20, 45, 70), (37, 18, 33)])
+@pytest.mark.parametrize("shape", [(7, 6, 5), (20, 45, 70), (37, 18, 33), (20, 45, 72), (37, 18, 36), (26, 50, 100)])
 def test_correct_intensity(disc, oracle_mod, shape, R):
     m, s = rand_pair(shape, 30 + R)
     ctx = make_ctx(disc, shape, R=R)
@@ -135,7 +138,8 @@ def test_force_update(disc, oracle_mod, shape):
 
 
 @pytest.mark.parametrize("sigma", [0.3, 1.0, 1.5, 2.0, 2.5, 3.0, 4.0])
-@pytest.mark.parametrize("shape", [(7, 6, 5), (20, 45, 70), (32, 64, 64), (3, 40, 2), (40, 300, 150)])
+@pytest.mark.parametrize("shape", [(7, 6, 5), (20, 45, 70), (32, 64, 64), (3, 40, 2), (40, 300, 150), (20, 45, 72),
+                                   (33, 70, 260)])
 def test_smooth_field(disc, oracle_mod, shape, sigma):
     r0 = np.random.default_rng(50).normal(0, 3, size=(3,) + shape).astype(np.float32)
     ctx = make_ctx(disc, shape, sigma=sigma)
