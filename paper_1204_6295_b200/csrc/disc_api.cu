@@ -39,6 +39,7 @@ struct disc_ctx {
     float sigma;
     int levels, iters;
     int K;
+    int n_sm;
     GaussTaps taps;
     Level lv[DISC_MAX_LEVELS];
     float* h2d_ct;    // device staging for disc_register_host
@@ -97,13 +98,35 @@ int pick_chunk(int n, int min_chunk, long long ctas_per_chunk, long long target_
 }
 
 // ------------------------------------------------------------------ kernels instantiated in moments_tu.cu / field_tu.cu
+// Tile height and z chunk of the moments kernel: minimise (waves) x (slices marched per CTA, with the 2R halo)
+// x (rows per slice, with the x pass's 2R halo rows).  The 32x32 tile runs one CTA per SM, the 32x16 tile two.
+void pick_moments_shape(const disc_ctx* c, const Level& L, int* ty_out, int* zchunk_out) {
+    const int R = c->R;
+    double best = 1e300;
+    int best_ty = 16, best_zc = L.nz;
+    for (int ty = 16; ty <= 32; ty += 16) {
+        if (ty == 32 && R > kMomMaxRTile32) continue;
+        const long long tiles = (long long)((L.nx + 31) / 32) * ((L.ny + ty - 1) / ty);
+        const long long slots = (long long)c->n_sm * (ty == 16 ? 2 : 1);
+        for (int nchunk = 1; nchunk <= L.nz; ++nchunk) {
+            const int zc = (L.nz + nchunk - 1) / nchunk;
+            const long long ctas = tiles * ((L.nz + zc - 1) / zc);
+            const long long waves = (ctas + slots - 1) / slots;
+            const double cost = (double)waves * (zc + 2 * R + 6) * (ty + R + 4) * (ty == 16 ? 1.6 : 1.0);
+            if (cost < best) { best = cost; best_ty = ty; best_zc = zc; }
+            if (zc == 1) break;
+        }
+    }
+    *ty_out = tune("DISC_TUNE_MOM_TY", best_ty);
+    *zchunk_out = tune("DISC_TUNE_MOM_ZCHUNK", best_zc);
+}
+
 template <int MODE>
 disc_status launch_moments(disc_ctx* c, const Level& L, const float* vol, const float* aux, float* out0,
                            float* out1, cudaStream_t st) {
-    const int tiles = ((L.nx + kMomTX - 1) / kMomTX) * ((L.ny + kMomTY - 1) / kMomTY);
-    const int W = 2 * c->R + 1;
-    const int zchunk = tune("DISC_TUNE_MOM_ZCHUNK", pick_chunk(L.nz, 4 * W > 32 ? 4 * W : 32, tiles, 2 * 148));
-    if (!launch_moments_any(c->R, MODE, vol, aux, out0, out1, L.nx, L.ny, L.nz, zchunk, DISC_EPS_VAR, st))
+    int ty, zchunk;
+    pick_moments_shape(c, L, &ty, &zchunk);
+    if (!launch_moments_any(c->R, MODE, ty, vol, aux, out0, out1, L.nx, L.ny, L.nz, zchunk, DISC_EPS_VAR, st))
         return fail(c, DISC_ERR_UNSUPPORTED, "patch_radius %d > %d", c->R, DISC_MAX_PATCH_RADIUS);
     return check_launch(c, "k_moments");
 }
@@ -214,6 +237,8 @@ disc_status disc_create(disc_ctx** out, const int dims[3], const float spacing[3
     if (!c) return fail(nullptr, DISC_ERR_ALLOC, "out of host memory");
     std::memset(c, 0, sizeof(*c));
     for (int i = 0; i < 3; ++i) { c->dims[i] = dims[i]; c->spacing[i] = spacing[i]; }
+    c->n_sm = 148;
+    cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
     c->R = patch_radius; c->sigma = sigma_smooth; c->levels = levels; c->iters = iters; c->K = K;
     // Gaussian taps: fp64, normalised to sum 1, then rounded to fp32 (reading A10)
     {

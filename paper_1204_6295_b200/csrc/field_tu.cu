@@ -56,20 +56,39 @@ static void launch_gz(const float* rin, float* rout, const float* moving, float*
     k_gz_warp<K, WARP><<<grid, 128, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps);
 }
 
-#define DISC_IN(k) ((k) >= DISC_K_LO && (k) <= DISC_K_HI)
-#define DISC_KK(k) (DISC_IN(k) ? (k) : DISC_K_LO)
+// one Gaussian radius: launches if K lies in this unit's range (the discarded branch is never instantiated)
+template <int K>
+static bool case_fg(bool force, int txb, const float* m, const float* s, const float* rin, float* rout, int nx, int ny,
+                    int nz, int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
+    if constexpr (K >= DISC_K_LO && K <= DISC_K_HI) {
+        if (force) launch_fg<K, true>(txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
+        else launch_fg<K, false>(txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
+        return true;
+    } else {
+        return false;
+    }
+}
+
+template <int K>
+static bool case_gz(bool warp, const float* rin, float* rout, const float* moving, float* mout, int nx, int ny, int nz,
+                    int zchunk, const GaussTaps& taps, cudaStream_t st) {
+    if constexpr (K >= DISC_K_LO && K <= DISC_K_HI) {
+        if (warp) launch_gz<K, true>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st);
+        else launch_gz<K, false>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st);
+        return true;
+    } else {
+        return false;
+    }
+}
+
 #define DISC_FOR_K(X) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12)
 
 bool DISC_CAT(launch_force_gxy_tu, DISC_TU)(int K, bool force, int txb, const float* m, const float* s,
                                             const float* rin, float* rout, int nx, int ny, int nz, int yseg,
                                             float eps_den, const GaussTaps& taps, cudaStream_t st) {
     switch (K) {
-#define DISC_CASE(k)                                                                                       \
-    case k:                                                                                                \
-        if (!DISC_IN(k)) return false;                                                                     \
-        if (force) launch_fg<DISC_KK(k), true>(txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);  \
-        else launch_fg<DISC_KK(k), false>(txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);       \
-        return true;
+#define DISC_CASE(k) \
+    case k: return case_fg<k>(force, txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
         DISC_FOR_K(DISC_CASE)
 #undef DISC_CASE
     }
@@ -80,12 +99,8 @@ bool DISC_CAT(launch_gz_warp_tu, DISC_TU)(int K, bool warp, const float* rin, fl
                                           float* mout, int nx, int ny, int nz, int zchunk, const GaussTaps& taps,
                                           cudaStream_t st) {
     switch (K) {
-#define DISC_CASE(k)                                                                                 \
-    case k:                                                                                          \
-        if (!DISC_IN(k)) return false;                                                               \
-        if (warp) launch_gz<DISC_KK(k), true>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st); \
-        else launch_gz<DISC_KK(k), false>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st);     \
-        return true;
+#define DISC_CASE(k) \
+    case k: return case_gz<k>(warp, rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st);
         DISC_FOR_K(DISC_CASE)
 #undef DISC_CASE
     }
@@ -104,12 +119,12 @@ void launch_warp_kernel(const float* moving, const float* r, float* out, int nx,
     k_warp<<<grid, 256, 0, st>>>(moving, r, out, nx, ny, nz);
 }
 
-bool launch_moments_any(int R, int mode, const float* vol, const float* aux, float* out0, float* out1, int nx,
+bool launch_moments_any(int R, int mode, int ty, const float* vol, const float* aux, float* out0, float* out1, int nx,
                         int ny, int nz, int zchunk, float eps_var, cudaStream_t st) {
-    return launch_moments_tu0(R, mode, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st) ||
-           launch_moments_tu1(R, mode, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st) ||
-           launch_moments_tu2(R, mode, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st) ||
-           launch_moments_tu3(R, mode, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st);
+    return launch_moments_tu0(R, mode, ty, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st) ||
+           launch_moments_tu1(R, mode, ty, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st) ||
+           launch_moments_tu2(R, mode, ty, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st) ||
+           launch_moments_tu3(R, mode, ty, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st);
 }
 
 bool launch_force_gxy_any(int K, bool force, int txb, const float* m, const float* s, const float* rin, float* rout,

@@ -9,7 +9,8 @@
 
 namespace disc {
 
-constexpr int kMomTX = 32, kMomTY = 16;  // (x,y) tile of the moments kernel
+constexpr int kMomTX = 32, kMomTY = 16;  // (x,y) tile of the plain-load moments kernel
+constexpr int kMomMaxRTile32 = 7;        // largest R whose z ring fits tensor memory with the 32x32 tile (moments_v2.cuh)
 
 enum MomentsMode {
     kModeMoments = 0,  // out0 = mean, out1 = var                                   (disc_box_moments)
@@ -18,7 +19,7 @@ enum MomentsMode {
 };
 
 
-bool launch_moments_any(int R, int mode, const float* vol, const float* aux, float* out0, float* out1, int nx,
+bool launch_moments_any(int R, int mode, int ty, const float* vol, const float* aux, float* out0, float* out1, int nx,
                         int ny, int nz, int zchunk, float eps_var, cudaStream_t st);
 bool launch_force_gxy_any(int K, bool force, int txb, const float* m, const float* s, const float* rin, float* rout,
                           int nx, int ny, int nz, int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st);
@@ -30,7 +31,7 @@ void launch_warp_kernel(const float* moving, const float* r, float* out, int nx,
 
 // per-translation-unit entry points (defined by moments_tu.cu / field_tu.cu with -DDISC_TU=n)
 #define DISC_DECL_TU(n)                                                                                                  \
-    bool launch_moments_tu##n(int R, int mode, const float* vol, const float* aux, float* out0, float* out1, int nx,     \
+    bool launch_moments_tu##n(int R, int mode, int ty, const float* vol, const float* aux, float* out0, float* out1, int nx,     \
                               int ny, int nz, int zchunk, float eps_var, cudaStream_t st);                              \
     bool launch_force_gxy_tu##n(int K, bool force, int txb, const float* m, const float* s, const float* rin,           \
                                 float* rout, int nx, int ny, int nz, int yseg, float eps_den, const GaussTaps& taps,    \
