@@ -1,7 +1,10 @@
 // field_tu.cu -- instantiates k_force_gxy<K,...> and k_gz_warp<K,...> for K in [DISC_K_LO, DISC_K_HI]; built
 // once per range (-DDISC_TU=n -DDISC_K_LO=a -DDISC_K_HI=b).  TU 0 also holds the K-independent kernels.
+#include <cstdlib>
+
 #include "field.cuh"
 #include "field_tma.cuh"
+#include "field_v2.cuh"
 #include "launch.h"
 
 #define DISC_CAT2(a, b) a##b
@@ -27,6 +30,17 @@ static void launch_fg_tma(const float* m, const float* s, const float* rin, floa
 template <int K, bool FORCE>
 static void launch_fg(int txb, const float* m, const float* s, const float* rin, float* rout, int nx, int ny, int nz,
                       int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
+    if (nx % 4 == 0 && aligned16(rout) && std::getenv("DISC_TUNE_FG_OLD") == nullptr) {
+        using C = FgTileCfg<K>;
+        static bool configured = false;  // one attribute call per instance (idempotent, so a race is harmless)
+        if (!configured) {
+            cudaFuncSetAttribute(k_force_gxy_tile<K, FORCE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
+            configured = true;
+        }
+        dim3 grid((nx + C::TX - 1) / C::TX, (ny + C::TY - 1) / C::TY, nz);
+        k_force_gxy_tile<K, FORCE><<<grid, C::NT, C::smem_bytes, st>>>(m, s, rin, rout, nx, ny, nz, eps_den, taps);
+        return;
+    }
     const bool tma_ok = nx % 4 == 0 && aligned16(rin) && aligned16(rout) && (!FORCE || (aligned16(m) && aligned16(s)));
     if (tma_ok) {
         if (nx > 128) launch_fg_tma<K, FORCE, 128>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
@@ -48,8 +62,14 @@ static void launch_gz(const float* rin, float* rout, const float* moving, float*
                       int zchunk, const GaussTaps& taps, cudaStream_t st) {
     const size_t plane = (size_t)nx * ny;
     if (nx % 4 == 0 && aligned16(rin) && aligned16(rout) && (!WARP || aligned16(mout))) {
-        dim3 grid((unsigned)((plane + kGzCols - 1) / kGzCols), (nz + zchunk - 1) / zchunk, 1);
-        k_gz_warp_tma<K, WARP><<<grid, 128, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps);
+        static const bool two = std::getenv("DISC_TUNE_GZ_C2") != nullptr;
+        if (two) {
+            dim3 grid((unsigned)((plane + kGz2Cols - 1) / kGz2Cols), (nz + zchunk - 1) / zchunk, 1);
+            k_gz_warp_v2<K, WARP><<<grid, kGz2Threads, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps);
+        } else {
+            dim3 grid((unsigned)((plane + kGz1Threads - 1) / kGz1Threads), (nz + zchunk - 1) / zchunk, 1);
+            k_gz_warp_c1<K, WARP><<<grid, kGz1Threads, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps);
+        }
         return;
     }
     dim3 grid((unsigned)((plane + 127) / 128), (nz + zchunk - 1) / zchunk, 1);
