@@ -330,7 +330,9 @@ struct FgTileCfg {
     static constexpr int P2_TASKS = 3 * PY * (TX / LX);
     static constexpr int P3_TASKS = 3 * (TX / 4) * (TY / LY);
     static constexpr size_t smem_bytes = sizeof(float) * 3 * PY * (UP + XP);
-    static_assert(2 * K <= 24 && (LX + 2 * K) % 4 == 0, "x-pass run must be whole float4 chunks");
+    static constexpr int NV = (LX + 2 * K + 3) / 4;              // float4 chunks of one x-pass run (the last may overhang
+                                                                 // into the row's padding: g*LX + 4*NV <= UP)
+    static_assert(2 * K <= 24 && (TX - LX) + 4 * NV <= UP, "x-pass run must stay inside the padded U row");
 };
 
 template <int K, bool FORCE>
@@ -363,9 +365,9 @@ k_force_gxy_tile(const float* __restrict__ m, const float* __restrict__ s, const
     for (int t = tid; t < C::P2_TASKS; t += NT) {
         const int r = t % PY, q = t / PY, g = q % (TX / LX), cc = q / (TX / LX);
         const float4* up = reinterpret_cast<const float4*>(U + (cc * PY + r) * UP + g * LX);
-        float v[LX + 2 * K];
+        float v[4 * C::NV];
 #pragma unroll
-        for (int i = 0; i < (LX + 2 * K) / 4; ++i) {
+        for (int i = 0; i < C::NV; ++i) {
             const float4 f = up[i];
             v[4 * i] = f.x; v[4 * i + 1] = f.y; v[4 * i + 2] = f.z; v[4 * i + 3] = f.w;
         }
