@@ -146,17 +146,13 @@ disc_status launch_force_gxy(disc_ctx* c, const Level& L, const float* m, const 
 template <bool WARP>
 disc_status launch_gz_warp(disc_ctx* c, const Level& L, const float* rin, float* rout, const float* moving,
                            float* mout, cudaStream_t st) {
-    // CTAs of 128 columns march a z chunk (plus the 2K halo slices).  One wave: as many chunks as keep every CTA
-    // resident (7 CTAs of 64 threads per SM), but no chunk shorter than 4K slices.
-    const size_t plane = (size_t)L.nx * L.ny;
-    const long long bx = (long long)((plane + 127) / 128);
+    // a thread owns one column and `lz` output slices (field_v3.cuh); fewer slices per thread while the level is too
+    // small to fill the SMs otherwise (the extra re-reads of the 2K halo slices then come from L2 anyway)
     const int K = c->K;
-    long long nchunk = (7LL * c->n_sm) / bx;
-    if (nchunk < 1) nchunk = 1;
-    int zchunk = (int)((L.nz + nchunk - 1) / nchunk);
-    if (zchunk < 4 * K) zchunk = 4 * K;
-    if (zchunk > L.nz) zchunk = L.nz;
-    zchunk = tune("DISC_TUNE_GZ_ZCHUNK", zchunk);
+    int lz = (long long)L.N / 8 >= 1024LL * c->n_sm ? 8 : 4;
+    lz = tune("DISC_TUNE_GZ_LZ", lz);
+    const int cols = tune("DISC_TUNE_GZ_COLS", 2);   // columns per thread: 2 = packed (needs nx even), 1 = scalar
+    const int zchunk = lz + 100 * cols;
     if (!launch_gz_warp_any(K, WARP, rin, rout, moving, mout, L.nx, L.ny, L.nz, zchunk, c->taps, st))
         return fail(c, DISC_ERR_UNSUPPORTED, "Gaussian radius %d unsupported", K);
     return check_launch(c, "k_gz_warp");

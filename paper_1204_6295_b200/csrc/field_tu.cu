@@ -3,8 +3,8 @@
 #include <cstdlib>
 
 #include "field.cuh"
-#include "field_tma.cuh"
 #include "field_v2.cuh"
+#include "field_v3.cuh"
 #include "launch.h"
 
 #define DISC_CAT2(a, b) a##b
@@ -14,38 +14,18 @@ namespace disc {
 
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-template <int K, bool FORCE, int NT>
-static void launch_fg_tma(const float* m, const float* s, const float* rin, float* rout, int nx, int ny, int nz,
-                          int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
-    using C = FgCfg<K, FORCE, NT>;
-    static bool configured = false;  // one attribute call per instance (idempotent, so a race is harmless)
-    if (!configured) {
-        cudaFuncSetAttribute(k_force_gxy_tma<K, FORCE, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
-        configured = true;
-    }
-    dim3 grid((nx + C::TX - 1) / C::TX, (ny + yseg - 1) / yseg, nz);
-    k_force_gxy_tma<K, FORCE, NT><<<grid, NT, C::smem_bytes, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps);
-}
-
 template <int K, bool FORCE>
 static void launch_fg(int txb, const float* m, const float* s, const float* rin, float* rout, int nx, int ny, int nz,
                       int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
-    if (nx % 4 == 0 && aligned16(rout) && std::getenv("DISC_TUNE_FG_OLD") == nullptr) {
-        using C = FgTileCfg<K>;
+    if (nx % 4 == 0 && aligned16(rin) && aligned16(rout) && (!FORCE || (aligned16(m) && aligned16(s)))) {
+        using C = FgT4Cfg<K>;
         static bool configured = false;  // one attribute call per instance (idempotent, so a race is harmless)
         if (!configured) {
-            cudaFuncSetAttribute(k_force_gxy_tile<K, FORCE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
+            cudaFuncSetAttribute(k_force_gxy_t4<K, FORCE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
             configured = true;
         }
         dim3 grid((nx + C::TX - 1) / C::TX, (ny + C::TY - 1) / C::TY, nz);
-        k_force_gxy_tile<K, FORCE><<<grid, C::NT, C::smem_bytes, st>>>(m, s, rin, rout, nx, ny, nz, eps_den, taps);
-        return;
-    }
-    const bool tma_ok = nx % 4 == 0 && aligned16(rin) && aligned16(rout) && (!FORCE || (aligned16(m) && aligned16(s)));
-    if (tma_ok) {
-        if (nx > 128) launch_fg_tma<K, FORCE, 128>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
-        else if (nx > 64) launch_fg_tma<K, FORCE, 64>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
-        else launch_fg_tma<K, FORCE, 32>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
+        k_force_gxy_t4<K, FORCE><<<grid, C::NT, C::smem_bytes, st>>>(m, s, rin, rout, nx, ny, nz, eps_den, taps);
         return;
     }
     dim3 grid((nx + txb - 1) / txb, (ny + yseg - 1) / yseg, nz);
@@ -57,23 +37,36 @@ static void launch_fg(int txb, const float* m, const float* s, const float* rin,
         k_force_gxy<K, FORCE, 32><<<grid, 32, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps);
 }
 
+template <int K, bool WARP, int LZ>
+static void launch_gzd(const float* rin, float* rout, const float* moving, float* mout, int nx, int ny, int nz,
+                       const GaussTaps& taps, cudaStream_t st) {
+    const size_t plane = (size_t)nx * ny;
+    dim3 grid((unsigned)((plane + kGzdThreads - 1) / kGzdThreads), (nz + LZ - 1) / LZ, 1);
+    k_gz_warp_d<K, WARP, LZ><<<grid, kGzdThreads, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, taps);
+}
+
+template <int K, bool WARP, int LZ>
+static void launch_gzd2(const float* rin, float* rout, const float* moving, float* mout, int nx, int ny, int nz,
+                        const GaussTaps& taps, cudaStream_t st) {
+    const size_t pairs = (size_t)nx * ny / 2;
+    dim3 grid((unsigned)((pairs + kGzdThreads - 1) / kGzdThreads), (nz + LZ - 1) / LZ, 1);
+    k_gz_warp_d2<K, WARP, LZ><<<grid, kGzdThreads, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, taps);
+}
+
+static inline bool aligned8(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 7u) == 0; }
+
 template <int K, bool WARP>
 static void launch_gz(const float* rin, float* rout, const float* moving, float* mout, int nx, int ny, int nz,
                       int zchunk, const GaussTaps& taps, cudaStream_t st) {
-    const size_t plane = (size_t)nx * ny;
-    if (nx % 4 == 0 && aligned16(rin) && aligned16(rout) && (!WARP || aligned16(mout))) {
-        static const bool two = std::getenv("DISC_TUNE_GZ_C2") != nullptr;
-        if (two) {
-            dim3 grid((unsigned)((plane + kGz2Cols - 1) / kGz2Cols), (nz + zchunk - 1) / zchunk, 1);
-            k_gz_warp_v2<K, WARP><<<grid, kGz2Threads, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps);
-        } else {
-            dim3 grid((unsigned)((plane + kGz1Threads - 1) / kGz1Threads), (nz + zchunk - 1) / zchunk, 1);
-            k_gz_warp_c1<K, WARP><<<grid, kGz1Threads, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps);
-        }
+    // zchunk = output slices per thread (4 or 8) + 100 * (columns per thread, 1 or 2), chosen by the caller
+    const int lz = zchunk % 100, two = zchunk / 100 >= 2;
+    if (two && nx % 2 == 0 && aligned8(rin) && aligned8(rout) && (!WARP || aligned8(mout))) {
+        if (lz >= 8) launch_gzd2<K, WARP, 8>(rin, rout, moving, mout, nx, ny, nz, taps, st);
+        else launch_gzd2<K, WARP, 4>(rin, rout, moving, mout, nx, ny, nz, taps, st);
         return;
     }
-    dim3 grid((unsigned)((plane + 127) / 128), (nz + zchunk - 1) / zchunk, 1);
-    k_gz_warp<K, WARP><<<grid, 128, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps);
+    if (lz >= 8) launch_gzd<K, WARP, 8>(rin, rout, moving, mout, nx, ny, nz, taps, st);
+    else launch_gzd<K, WARP, 4>(rin, rout, moving, mout, nx, ny, nz, taps, st);
 }
 
 // one Gaussian radius: launches if K lies in this unit's range (the discarded branch is never instantiated)

@@ -1,0 +1,314 @@
+// field_v3.cuh -- third generation of the two field kernels (same arithmetic as field.cuh, same results up to
+// fp32 rounding order).  profiles/r01b showed both second-generation kernels bound by their INSTRUCTION COUNT
+// (280-290 thread instructions per voxel, a quarter of them pipeline bookkeeping and 64-bit address arithmetic)
+// and by the exposed latency of their loads.  Here:
+//
+//   k_gz_warp_d<K, WARP, LZ>   Gaussian z pass (+ warp).  No ring, no shared memory, no barriers: a thread owns ONE
+//                              (x,y) column and LZ consecutive output slices; per component it issues all LZ + 2K
+//                              input loads at once (coalesced across the warp, latency overlapped LZ + 2K deep),
+//                              forms the LZ outputs with statically indexed registers, and then runs the warp's
+//                              trilinear gathers in batches of four voxels (32 independent loads in flight).
+//                              The input is re-read (LZ + 2K)/LZ times, but only from L2: neighbouring z blocks
+//                              run at the same time on other SMs.
+#pragma once
+#include "common.cuh"
+#include "field_v2.cuh"
+
+namespace disc {
+
+constexpr int kGzdThreads = 128;
+
+template <int K, bool WARP, int LZ>
+__global__ void __launch_bounds__(kGzdThreads)
+k_gz_warp_d(const float* __restrict__ rin, float* __restrict__ rout, const float* __restrict__ moving,
+            float* __restrict__ mout, int nx, int ny, int nz, GaussTaps gw) {
+    constexpr int W = 2 * K + 1, NV = LZ + 2 * K;
+    const unsigned plane = (unsigned)nx * (unsigned)ny;
+    const unsigned col = blockIdx.x * kGzdThreads + threadIdx.x;
+    if (col >= plane) return;
+    const size_t N = (size_t)plane * nz;
+    const int z0 = blockIdx.y * LZ;
+    const bool interior = z0 - K >= 0 && z0 + LZ + K <= nz;   // uniform over the CTA
+
+    float res[3][LZ];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float* src = rin + c * N + col;
+        float v[NV];
+        if (interior) {
+            const float* p = src + (size_t)(z0 - K) * plane;
+#pragma unroll
+            for (int i = 0; i < NV; ++i) v[i] = __ldg(p + (size_t)i * plane);
+        } else {
+#pragma unroll
+            for (int i = 0; i < NV; ++i) v[i] = __ldg(src + (size_t)clampi(z0 - K + i, 0, nz - 1) * plane);   // replicate border
+        }
+#pragma unroll
+        for (int j = 0; j < LZ; ++j) {
+            float acc = 0.f;
+#pragma unroll
+            for (int k = 0; k < W; ++k) acc = fmaf(gw.w[k], v[j + k], acc);
+            res[c][j] = acc;
+        }
+        float* dst = rout + c * N + (size_t)z0 * plane + col;
+        if (interior) {
+#pragma unroll
+            for (int j = 0; j < LZ; ++j) dst[(size_t)j * plane] = res[c][j];
+        } else {
+#pragma unroll
+            for (int j = 0; j < LZ; ++j)
+                if (z0 + j < nz) dst[(size_t)j * plane] = res[c][j];
+        }
+    }
+    if (WARP) {
+        const int y = (int)(col / (unsigned)nx), x = (int)(col - (unsigned)y * (unsigned)nx);
+        const float fx = (float)x, fy = (float)y;
+        const bool fast = nx > 1 && ny > 1 && nz > 1 && N < (size_t)0x7fffffff;   // 32-bit voxel indices
+        float* mp = mout + (size_t)z0 * plane + col;
+        constexpr int B = 4;
+        static_assert(LZ % B == 0, "gather batches");
+#pragma unroll
+        for (int j0 = 0; j0 < LZ; j0 += B) {
+            TriSample g[B];
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                const int j = j0 + b;
+                const float fz = (float)(z0 + j);
+                if (fast) tri_issue<true>(moving, nx, ny, nz, fx + res[0][j], fy + res[1][j], fz + res[2][j], g[b]);
+                else tri_issue<false>(moving, nx, ny, nz, fx + res[0][j], fy + res[1][j], fz + res[2][j], g[b]);
+            }
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                const int j = j0 + b;
+                const float mv = tri_finish(g[b]);
+                if (interior || z0 + j < nz) mp[(size_t)j * plane] = mv;
+            }
+        }
+    }
+}
+
+// Two adjacent columns per thread (nx even, 8-byte aligned fields): 8-byte loads and stores, packed FFMA2 taps --
+// half the load / store / FMA instructions and half the address arithmetic per voxel.
+template <int K, bool WARP, int LZ>
+__global__ void __launch_bounds__(kGzdThreads)
+k_gz_warp_d2(const float* __restrict__ rin, float* __restrict__ rout, const float* __restrict__ moving,
+             float* __restrict__ mout, int nx, int ny, int nz, GaussTaps gw) {
+    constexpr int W = 2 * K + 1, NV = LZ + 2 * K;
+    const unsigned plane = (unsigned)nx * (unsigned)ny;
+    const unsigned col = 2u * (blockIdx.x * kGzdThreads + threadIdx.x);
+    if (col >= plane) return;
+    const size_t N = (size_t)plane * nz;
+    const int z0 = blockIdx.y * LZ;
+    const bool interior = z0 - K >= 0 && z0 + LZ + K <= nz;   // uniform over the CTA
+
+    float2 res[3][LZ];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float* src = rin + c * N + col;
+        float2 v[NV];
+        if (interior) {
+            const float* p = src + (size_t)(z0 - K) * plane;
+#pragma unroll
+            for (int i = 0; i < NV; ++i) { v[i] = __ldg(reinterpret_cast<const float2*>(p)); p += plane; }
+        } else {
+#pragma unroll
+            for (int i = 0; i < NV; ++i)
+                v[i] = __ldg(reinterpret_cast<const float2*>(src + (size_t)clampi(z0 - K + i, 0, nz - 1) * plane));   // replicate border
+        }
+#pragma unroll
+        for (int j = 0; j < LZ; ++j) {
+            float2 acc = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int k = 0; k < W; ++k) acc = ffma2(make_float2(gw.w[k], gw.w[k]), v[j + k], acc);
+            res[c][j] = acc;
+        }
+        float* dst = rout + c * N + (size_t)z0 * plane + col;
+#pragma unroll
+        for (int j = 0; j < LZ; ++j) {
+            if (interior || z0 + j < nz) *reinterpret_cast<float2*>(dst) = res[c][j];
+            dst += plane;
+        }
+    }
+    if (WARP) {
+        const int y = (int)(col / (unsigned)nx), x = (int)(col - (unsigned)y * (unsigned)nx);   // both columns share y (nx even)
+        const float fx0 = (float)x, fx1 = (float)(x + 1), fy = (float)y;
+        const bool fast = nx > 1 && ny > 1 && nz > 1 && N < (size_t)0x7fffffff;   // 32-bit voxel indices
+        float* mp = mout + (size_t)z0 * plane + col;
+        constexpr int B = 2;
+        static_assert(LZ % B == 0, "gather batches");
+#pragma unroll
+        for (int j0 = 0; j0 < LZ; j0 += B) {
+            TriSample g[B][2];
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                const int j = j0 + b;
+                const float fz = (float)(z0 + j);
+                if (fast) {
+                    tri_issue<true>(moving, nx, ny, nz, fx0 + res[0][j].x, fy + res[1][j].x, fz + res[2][j].x, g[b][0]);
+                    tri_issue<true>(moving, nx, ny, nz, fx1 + res[0][j].y, fy + res[1][j].y, fz + res[2][j].y, g[b][1]);
+                } else {
+                    tri_issue<false>(moving, nx, ny, nz, fx0 + res[0][j].x, fy + res[1][j].x, fz + res[2][j].x, g[b][0]);
+                    tri_issue<false>(moving, nx, ny, nz, fx1 + res[0][j].y, fy + res[1][j].y, fz + res[2][j].y, g[b][1]);
+                }
+            }
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                const int j = j0 + b;
+                const float2 mv = make_float2(tri_finish(g[b][0]), tri_finish(g[b][1]));
+                if (interior || z0 + j < nz) *reinterpret_cast<float2*>(mp) = mv;
+                mp += plane;
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// [force + update] + Gaussian x + Gaussian y, tile kernel with a VECTORISED phase 1.
+//
+// Same three phases as k_force_gxy_tile (field_v2.cuh), but phase 1 -- which held 70 % of that kernel's
+// instructions (profiles/r01b: 128 per point, 11 scalar loads each with its own 64-bit address) -- now works on
+// groups of four x-adjacent points: nine 16-byte loads and two scalar ones per group, one address computation per
+// load, one 16-byte store per component.  For that the tile's x halo is rounded out to a multiple of four
+// (KA = K rounded up), so every group is either wholly inside the volume or wholly outside it; outside groups are
+// the replicate border: the clamped point's value, broadcast.
+// Requirements (launcher): nx % 4 == 0, 16-byte aligned m, s, rin, rout.
+// ---------------------------------------------------------------------------------------------------------
+template <int K>
+struct FgT4Cfg {
+    static constexpr int TX = 64, TY = 32, NT = 256, LX = 8, LY = 8;
+    static constexpr int W = 2 * K + 1;
+    static constexpr int KA = (K + 3) / 4 * 4, OFF = KA - K;
+    static constexpr int PXA = TX + 2 * KA, PY = TY + 2 * K, NG = PXA / 4;
+    static constexpr int UP = ((PXA / 4) | 1) * 4;               // U row pitch: odd number of 16-byte chunks
+    static constexpr int XP = TX + 4;                            // X row pitch: 17 chunks (odd)
+    static constexpr int NV = (OFF + LX + 2 * K + 3) / 4;        // 16-byte chunks of one x-pass run
+    static constexpr int P2_TASKS = 3 * PY * (TX / LX);
+    static constexpr int P3_TASKS = 3 * (TX / 4) * (TY / LY);
+    static constexpr size_t smem_bytes = sizeof(float) * 3 * PY * (UP + XP);
+    static_assert((TX - LX) + 4 * NV <= UP, "x-pass run must stay inside the U row");
+};
+
+__device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+
+template <int K, bool FORCE>
+__global__ void __launch_bounds__(FgT4Cfg<K>::NT, 2)
+k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const float* __restrict__ rin,
+               float* __restrict__ rout, int nx, int ny, int nz, float eps_den, GaussTaps gw) {
+    using C = FgT4Cfg<K>;
+    constexpr int W = C::W, TX = C::TX, TY = C::TY, NT = C::NT, LX = C::LX, LY = C::LY, PY = C::PY, NG = C::NG;
+    constexpr int UP = C::UP, XP = C::XP, KA = C::KA, OFF = C::OFF, NV = C::NV;
+    extern __shared__ __align__(16) float smem_f[];
+    float* U = smem_f;                       // [3][PY][UP]
+    float* X = smem_f + 3 * PY * UP;         // [3][PY][XP]
+
+    const int tid = threadIdx.x;
+    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z = blockIdx.z;
+    const size_t plane = (size_t)nx * ny;
+    const size_t N = plane * nz;
+
+    // ---- phase 1: updated field at the tile + halo, four x-adjacent points at a time
+    for (int p = tid; p < PY * NG; p += NT) {
+        const int r = p / NG, g = p - r * NG;
+        const int gy = clampi(y0 - K + r, 0, ny - 1);
+        const int gx = x0 - KA + 4 * g;
+        float4 u[3];
+        if (gx >= 0 && gx < nx) {
+            const size_t i = (size_t)z * plane + (size_t)gy * nx + gx;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) u[c] = ldg4(rin + c * N + i);
+            if (FORCE) {
+                const float4 sc = ldg4(s + i), mm = ldg4(m + i);
+                const float sl = __ldg(s + i - (gx > 0 ? 1 : 0)), sr = __ldg(s + i + 3 + (gx + 4 < nx ? 1 : 0));
+                const float4 syp = ldg4(s + i + (gy < ny - 1 ? (size_t)nx : 0)), sym = ldg4(s + i - (gy > 0 ? (size_t)nx : 0));
+                const float4 szp = ldg4(s + i + (z < nz - 1 ? plane : 0)), szm = ldg4(s + i - (z > 0 ? plane : 0));
+                const float ce[6] = {sl, sc.x, sc.y, sc.z, sc.w, sr};
+                const float me[4] = {mm.x, mm.y, mm.z, mm.w};
+                const float yp[4] = {syp.x, syp.y, syp.z, syp.w}, ym[4] = {sym.x, sym.y, sym.z, sym.w};
+                const float zp[4] = {szp.x, szp.y, szp.z, szp.w}, zm[4] = {szm.x, szm.y, szm.z, szm.w};
+                float ux[4] = {u[0].x, u[0].y, u[0].z, u[0].w}, uy[4] = {u[1].x, u[1].y, u[1].z, u[1].w};
+                float uz[4] = {u[2].x, u[2].y, u[2].z, u[2].w};
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const float gxv = 0.5f * (ce[e + 2] - ce[e]);
+                    const float gyv = 0.5f * (yp[e] - ym[e]);
+                    const float gzv = 0.5f * (zp[e] - zm[e]);
+                    const float d = ce[e + 1] - me[e];
+                    const float den = fmaf(gxv, gxv, fmaf(gyv, gyv, fmaf(gzv, gzv, fmaf(d, d, eps_den))));
+                    const float q = __fdividef(d, den);
+                    ux[e] = fmaf(q, gxv, ux[e]);
+                    uy[e] = fmaf(q, gyv, uy[e]);
+                    uz[e] = fmaf(q, gzv, uz[e]);
+                }
+                u[0] = make_float4(ux[0], ux[1], ux[2], ux[3]);
+                u[1] = make_float4(uy[0], uy[1], uy[2], uy[3]);
+                u[2] = make_float4(uz[0], uz[1], uz[2], uz[3]);
+            }
+        } else {
+            // replicate border in x: the whole group lies outside the volume
+            float v[3];
+            updated_field<FORCE>(m, s, rin, nx, ny, nz, N, gx < 0 ? 0 : nx - 1, gy, z, eps_den, v);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) u[c] = make_float4(v[c], v[c], v[c], v[c]);
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) *reinterpret_cast<float4*>(U + (c * PY + r) * UP + 4 * g) = u[c];
+    }
+    __syncthreads();
+
+    // ---- phase 2: x pass, lanes <-> rows; output x0 + g*LX + j reads U columns OFF + g*LX + j + k
+    for (int t = tid; t < C::P2_TASKS; t += NT) {
+        const int r = t % PY, q = t / PY, g = q % (TX / LX), cc = q / (TX / LX);
+        const float4* up = reinterpret_cast<const float4*>(U + (cc * PY + r) * UP + g * LX);
+        float v[4 * NV];
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {
+            const float4 f = up[i];
+            v[4 * i] = f.x; v[4 * i + 1] = f.y; v[4 * i + 2] = f.z; v[4 * i + 3] = f.w;
+        }
+        float o[LX];
+#pragma unroll
+        for (int j = 0; j < LX; ++j) {
+            float acc = 0.f;
+#pragma unroll
+            for (int k = 0; k < W; ++k) acc = fmaf(gw.w[k], v[OFF + j + k], acc);
+            o[j] = acc;
+        }
+        float4* xp = reinterpret_cast<float4*>(X + (cc * PY + r) * XP + g * LX);
+        xp[0] = make_float4(o[0], o[1], o[2], o[3]);
+        xp[1] = make_float4(o[4], o[5], o[6], o[7]);
+    }
+    __syncthreads();
+
+    // ---- phase 3: y pass, lanes <-> column groups
+    for (int t = tid; t < C::P3_TASKS; t += NT) {
+        const int cg = t % (TX / 4), q = t / (TX / 4), h = q % (TY / LY), cc = q / (TY / LY);
+        const float4* xp = reinterpret_cast<const float4*>(X + (cc * PY + h * LY) * XP + cg * 4);
+        float2 a0[LY], a1[LY];
+#pragma unroll
+        for (int j = 0; j < LY; ++j) { a0[j] = make_float2(0.f, 0.f); a1[j] = make_float2(0.f, 0.f); }
+#pragma unroll
+        for (int i = 0; i < LY + 2 * K; ++i) {
+            const float4 f = xp[i * (XP / 4)];
+            const float2 lo = make_float2(f.x, f.y), hi = make_float2(f.z, f.w);
+#pragma unroll
+            for (int j = 0; j < LY; ++j) {
+                const int k = i - j;          // input row i contributes to output row j with tap k
+                if (k >= 0 && k < W) {
+                    const float2 w2 = make_float2(gw.w[k], gw.w[k]);
+                    a0[j] = ffma2(w2, lo, a0[j]);
+                    a1[j] = ffma2(w2, hi, a1[j]);
+                }
+            }
+        }
+        const int gx = x0 + cg * 4;
+        if (gx < nx) {
+            float* op = rout + cc * N + ((size_t)z * ny + (y0 + h * LY)) * nx + gx;
+#pragma unroll
+            for (int j = 0; j < LY; ++j)
+                if (y0 + h * LY + j < ny)
+                    *reinterpret_cast<float4*>(op + (size_t)j * nx) = make_float4(a0[j].x, a0[j].y, a1[j].x, a1[j].y);
+        }
+    }
+}
+
+}  // namespace disc
