@@ -18,7 +18,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libdisc.so")
 
 # no --use_fast_math: IEEE division and sqrt are kept
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
+NVCC_FLAGS = os.environ.get("DISC_EXTRA_FLAGS", "").split() + ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 R_RANGES = [(0, 3), (4, 5), (6, 7), (8, 10)]
 K_RANGES = [(1, 3), (4, 6), (7, 9), (10, 12)]

@@ -146,11 +146,10 @@ disc_status launch_force_gxy(disc_ctx* c, const Level& L, const float* m, const 
 template <bool WARP>
 disc_status launch_gz_warp(disc_ctx* c, const Level& L, const float* rin, float* rout, const float* moving,
                            float* mout, cudaStream_t st) {
-    // a thread owns one column and `lz` output slices (field_v3.cuh); fewer slices per thread while the level is too
-    // small to fill the SMs otherwise (the extra re-reads of the 2K halo slices then come from L2 anyway)
+    // a thread owns two adjacent columns and `lz` output slices (field_v3.cuh); measured on B200: with two columns
+    // per thread 4 slices beat 8 at every level (more threads in flight; the 2K halo re-reads come from L2)
     const int K = c->K;
-    int lz = (long long)L.N / 8 >= 1024LL * c->n_sm ? 8 : 4;
-    lz = tune("DISC_TUNE_GZ_LZ", lz);
+    const int lz = tune("DISC_TUNE_GZ_LZ", 4);
     const int cols = tune("DISC_TUNE_GZ_COLS", 2);   // columns per thread: 2 = packed (needs nx even), 1 = scalar
     const int zchunk = lz + 100 * cols;
     if (!launch_gz_warp_any(K, WARP, rin, rout, moving, mout, L.nx, L.ny, L.nz, zchunk, c->taps, st))

@@ -24,7 +24,14 @@ static void launch_fg(int txb, const float* m, const float* s, const float* rin,
             cudaFuncSetAttribute(k_force_gxy_t4<K, FORCE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
             configured = true;
         }
-        dim3 grid((nx + C::TX - 1) / C::TX, (ny + C::TY - 1) / C::TY, nz);
+        static int n_sm = 0;
+        if (!n_sm) {
+            int dev = 0;
+            cudaGetDevice(&dev);
+            cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        }
+        const long long n_tiles = (long long)((nx + C::TX - 1) / C::TX) * ((ny + C::TY - 1) / C::TY) * nz;
+        const int grid = (int)(n_tiles < (long long)C::OCC * n_sm ? n_tiles : (long long)C::OCC * n_sm);   // persistent: OCC CTAs per SM
         k_force_gxy_t4<K, FORCE><<<grid, C::NT, C::smem_bytes, st>>>(m, s, rin, rout, nx, ny, nz, eps_den, taps);
         return;
     }

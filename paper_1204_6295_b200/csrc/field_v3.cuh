@@ -173,9 +173,18 @@ k_gz_warp_d2(const float* __restrict__ rin, float* __restrict__ rout, const floa
 // the replicate border: the clamped point's value, broadcast.
 // Requirements (launcher): nx % 4 == 0, 16-byte aligned m, s, rin, rout.
 // ---------------------------------------------------------------------------------------------------------
+#ifndef DISC_FG_TY
+#define DISC_FG_TY 32
+#endif
+#ifndef DISC_FG_NT
+#define DISC_FG_NT 256
+#endif
+#ifndef DISC_FG_OCC
+#define DISC_FG_OCC 2
+#endif
 template <int K>
 struct FgT4Cfg {
-    static constexpr int TX = 64, TY = 32, NT = 256, LX = 8, LY = 8;
+    static constexpr int TX = 64, TY = DISC_FG_TY, NT = DISC_FG_NT, OCC = DISC_FG_OCC, LX = 8, LY = 8;
     static constexpr int W = 2 * K + 1;
     static constexpr int KA = (K + 3) / 4 * 4, OFF = KA - K;
     static constexpr int PXA = TX + 2 * KA, PY = TY + 2 * K, NG = PXA / 4;
@@ -190,8 +199,57 @@ struct FgT4Cfg {
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 
+// updated field of one group of four x-adjacent points (gx % 4 == 0), loads first, arithmetic after
+template <bool FORCE>
+struct FgGroup {
+    float4 u[3], sc, mm, syp, sym, szp, szm;
+    float sl, sr;
+    __device__ __forceinline__ void load(const float* __restrict__ m, const float* __restrict__ s,
+                                         const float* __restrict__ rin, int nx, int ny, int nz, size_t plane, size_t N,
+                                         int gx, int gy, int z) {
+        const size_t i = (size_t)z * plane + (size_t)gy * nx + gx;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) u[c] = ldg4(rin + c * N + i);
+        if (FORCE) {
+            sc = ldg4(s + i); mm = ldg4(m + i);
+            sl = __ldg(s + i - (gx > 0 ? 1 : 0)); sr = __ldg(s + i + 3 + (gx + 4 < nx ? 1 : 0));
+            syp = ldg4(s + i + (gy < ny - 1 ? (size_t)nx : 0)); sym = ldg4(s + i - (gy > 0 ? (size_t)nx : 0));
+            szp = ldg4(s + i + (z < nz - 1 ? plane : 0)); szm = ldg4(s + i - (z > 0 ? plane : 0));
+        }
+    }
+    __device__ __forceinline__ void finish(float eps_den) {
+        if (FORCE) {
+            const float ce[6] = {sl, sc.x, sc.y, sc.z, sc.w, sr};
+            const float me[4] = {mm.x, mm.y, mm.z, mm.w};
+            const float yp[4] = {syp.x, syp.y, syp.z, syp.w}, ym[4] = {sym.x, sym.y, sym.z, sym.w};
+            const float zp[4] = {szp.x, szp.y, szp.z, szp.w}, zm[4] = {szm.x, szm.y, szm.z, szm.w};
+            float ux[4] = {u[0].x, u[0].y, u[0].z, u[0].w}, uy[4] = {u[1].x, u[1].y, u[1].z, u[1].w};
+            float uz[4] = {u[2].x, u[2].y, u[2].z, u[2].w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const float gxv = 0.5f * (ce[e + 2] - ce[e]);
+                const float gyv = 0.5f * (yp[e] - ym[e]);
+                const float gzv = 0.5f * (zp[e] - zm[e]);
+                const float d = ce[e + 1] - me[e];
+                const float den = fmaf(gxv, gxv, fmaf(gyv, gyv, fmaf(gzv, gzv, fmaf(d, d, eps_den))));
+                const float q = __fdividef(d, den);
+                ux[e] = fmaf(q, gxv, ux[e]);
+                uy[e] = fmaf(q, gyv, uy[e]);
+                uz[e] = fmaf(q, gzv, uz[e]);
+            }
+            u[0] = make_float4(ux[0], ux[1], ux[2], ux[3]);
+            u[1] = make_float4(uy[0], uy[1], uy[2], uy[3]);
+            u[2] = make_float4(uz[0], uz[1], uz[2], uz[3]);
+        }
+    }
+};
+
+// PERSISTENT: the grid is two CTAs per SM; a CTA walks tiles t = blockIdx.x, += gridDim.x (x fastest, so the CTAs
+// running at the same time work on neighbouring tiles and share their halos in L2).  Phase 3 of tile t-1 and
+// phase 1 of tile t share one barrier interval -- the y pass (pure FMA work out of shared memory) runs on some
+// warps while others wait for phase 1's global loads.
 template <int K, bool FORCE>
-__global__ void __launch_bounds__(FgT4Cfg<K>::NT, 2)
+__global__ void __launch_bounds__(FgT4Cfg<K>::NT, FgT4Cfg<K>::OCC)
 k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const float* __restrict__ rin,
                float* __restrict__ rout, int nx, int ny, int nz, float eps_den, GaussTaps gw) {
     using C = FgT4Cfg<K>;
@@ -202,112 +260,96 @@ k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const f
     float* X = smem_f + 3 * PY * UP;         // [3][PY][XP]
 
     const int tid = threadIdx.x;
-    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z = blockIdx.z;
     const size_t plane = (size_t)nx * ny;
     const size_t N = plane * nz;
+    const int ntx = (nx + TX - 1) / TX, nty = (ny + TY - 1) / TY;
+    const int n_tiles = ntx * nty * nz;
 
-    // ---- phase 1: updated field at the tile + halo, four x-adjacent points at a time
-    for (int p = tid; p < PY * NG; p += NT) {
-        const int r = p / NG, g = p - r * NG;
-        const int gy = clampi(y0 - K + r, 0, ny - 1);
-        const int gx = x0 - KA + 4 * g;
-        float4 u[3];
-        if (gx >= 0 && gx < nx) {
-            const size_t i = (size_t)z * plane + (size_t)gy * nx + gx;
-#pragma unroll
-            for (int c = 0; c < 3; ++c) u[c] = ldg4(rin + c * N + i);
-            if (FORCE) {
-                const float4 sc = ldg4(s + i), mm = ldg4(m + i);
-                const float sl = __ldg(s + i - (gx > 0 ? 1 : 0)), sr = __ldg(s + i + 3 + (gx + 4 < nx ? 1 : 0));
-                const float4 syp = ldg4(s + i + (gy < ny - 1 ? (size_t)nx : 0)), sym = ldg4(s + i - (gy > 0 ? (size_t)nx : 0));
-                const float4 szp = ldg4(s + i + (z < nz - 1 ? plane : 0)), szm = ldg4(s + i - (z > 0 ? plane : 0));
-                const float ce[6] = {sl, sc.x, sc.y, sc.z, sc.w, sr};
-                const float me[4] = {mm.x, mm.y, mm.z, mm.w};
-                const float yp[4] = {syp.x, syp.y, syp.z, syp.w}, ym[4] = {sym.x, sym.y, sym.z, sym.w};
-                const float zp[4] = {szp.x, szp.y, szp.z, szp.w}, zm[4] = {szm.x, szm.y, szm.z, szm.w};
-                float ux[4] = {u[0].x, u[0].y, u[0].z, u[0].w}, uy[4] = {u[1].x, u[1].y, u[1].z, u[1].w};
-                float uz[4] = {u[2].x, u[2].y, u[2].z, u[2].w};
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const float gxv = 0.5f * (ce[e + 2] - ce[e]);
-                    const float gyv = 0.5f * (yp[e] - ym[e]);
-                    const float gzv = 0.5f * (zp[e] - zm[e]);
-                    const float d = ce[e + 1] - me[e];
-                    const float den = fmaf(gxv, gxv, fmaf(gyv, gyv, fmaf(gzv, gzv, fmaf(d, d, eps_den))));
-                    const float q = __fdividef(d, den);
-                    ux[e] = fmaf(q, gxv, ux[e]);
-                    uy[e] = fmaf(q, gyv, uy[e]);
-                    uz[e] = fmaf(q, gzv, uz[e]);
-                }
-                u[0] = make_float4(ux[0], ux[1], ux[2], ux[3]);
-                u[1] = make_float4(uy[0], uy[1], uy[2], uy[3]);
-                u[2] = make_float4(uz[0], uz[1], uz[2], uz[3]);
-            }
-        } else {
-            // replicate border in x: the whole group lies outside the volume
-            float v[3];
-            updated_field<FORCE>(m, s, rin, nx, ny, nz, N, gx < 0 ? 0 : nx - 1, gy, z, eps_den, v);
-#pragma unroll
-            for (int c = 0; c < 3; ++c) u[c] = make_float4(v[c], v[c], v[c], v[c]);
-        }
-#pragma unroll
-        for (int c = 0; c < 3; ++c) *reinterpret_cast<float4*>(U + (c * PY + r) * UP + 4 * g) = u[c];
-    }
-    __syncthreads();
+    int px0 = 0, py0 = 0, pz = 0;   // the previous tile (whose y pass is still due)
+    bool have_prev = false;
+    for (int t = blockIdx.x;; t += gridDim.x) {
+        const bool have = t < n_tiles;
+        const int z = t / (ntx * nty), txy = t - z * (ntx * nty);
+        const int y0 = (txy / ntx) * TY, x0 = (txy - (txy / ntx) * ntx) * TX;
 
-    // ---- phase 2: x pass, lanes <-> rows; output x0 + g*LX + j reads U columns OFF + g*LX + j + k
-    for (int t = tid; t < C::P2_TASKS; t += NT) {
-        const int r = t % PY, q = t / PY, g = q % (TX / LX), cc = q / (TX / LX);
-        const float4* up = reinterpret_cast<const float4*>(U + (cc * PY + r) * UP + g * LX);
-        float v[4 * NV];
+        // ---- phase 1 of tile t: updated field at the tile + halo, four x-adjacent points at a time
+        if (have) {
+            for (int p = tid; p < PY * NG; p += NT) {
+                const int r = p / NG, g = p - r * NG;
+                const int gy = clampi(y0 - K + r, 0, ny - 1);
+                const int gx = x0 - KA + 4 * g;
+                // a group wholly outside the volume is the replicate border: the edge group's outermost value
+                FgGroup<FORCE> G;
+                G.load(m, s, rin, nx, ny, nz, plane, N, clampi(gx, 0, nx - 4), gy, z);
+                G.finish(eps_den);
 #pragma unroll
-        for (int i = 0; i < NV; ++i) {
-            const float4 f = up[i];
-            v[4 * i] = f.x; v[4 * i + 1] = f.y; v[4 * i + 2] = f.z; v[4 * i + 3] = f.w;
-        }
-        float o[LX];
-#pragma unroll
-        for (int j = 0; j < LX; ++j) {
-            float acc = 0.f;
-#pragma unroll
-            for (int k = 0; k < W; ++k) acc = fmaf(gw.w[k], v[OFF + j + k], acc);
-            o[j] = acc;
-        }
-        float4* xp = reinterpret_cast<float4*>(X + (cc * PY + r) * XP + g * LX);
-        xp[0] = make_float4(o[0], o[1], o[2], o[3]);
-        xp[1] = make_float4(o[4], o[5], o[6], o[7]);
-    }
-    __syncthreads();
-
-    // ---- phase 3: y pass, lanes <-> column groups
-    for (int t = tid; t < C::P3_TASKS; t += NT) {
-        const int cg = t % (TX / 4), q = t / (TX / 4), h = q % (TY / LY), cc = q / (TY / LY);
-        const float4* xp = reinterpret_cast<const float4*>(X + (cc * PY + h * LY) * XP + cg * 4);
-        float2 a0[LY], a1[LY];
-#pragma unroll
-        for (int j = 0; j < LY; ++j) { a0[j] = make_float2(0.f, 0.f); a1[j] = make_float2(0.f, 0.f); }
-#pragma unroll
-        for (int i = 0; i < LY + 2 * K; ++i) {
-            const float4 f = xp[i * (XP / 4)];
-            const float2 lo = make_float2(f.x, f.y), hi = make_float2(f.z, f.w);
-#pragma unroll
-            for (int j = 0; j < LY; ++j) {
-                const int k = i - j;          // input row i contributes to output row j with tap k
-                if (k >= 0 && k < W) {
-                    const float2 w2 = make_float2(gw.w[k], gw.w[k]);
-                    a0[j] = ffma2(w2, lo, a0[j]);
-                    a1[j] = ffma2(w2, hi, a1[j]);
+                for (int c = 0; c < 3; ++c) {
+                    float4 v = G.u[c];
+                    if (gx < 0) v = make_float4(v.x, v.x, v.x, v.x);
+                    else if (gx >= nx) v = make_float4(v.w, v.w, v.w, v.w);
+                    *reinterpret_cast<float4*>(U + (c * PY + r) * UP + 4 * g) = v;
                 }
             }
         }
-        const int gx = x0 + cg * 4;
-        if (gx < nx) {
-            float* op = rout + cc * N + ((size_t)z * ny + (y0 + h * LY)) * nx + gx;
+        // ---- phase 3 of tile t-1: y pass, lanes <-> column groups
+        if (have_prev) {
+            for (int tk = tid; tk < C::P3_TASKS; tk += NT) {
+                const int cg = tk % (TX / 4), q = tk / (TX / 4), h = q % (TY / LY), cc = q / (TY / LY);
+                const float4* xp = reinterpret_cast<const float4*>(X + (cc * PY + h * LY) * XP + cg * 4);
+                float2 a0[LY], a1[LY];
 #pragma unroll
-            for (int j = 0; j < LY; ++j)
-                if (y0 + h * LY + j < ny)
-                    *reinterpret_cast<float4*>(op + (size_t)j * nx) = make_float4(a0[j].x, a0[j].y, a1[j].x, a1[j].y);
+                for (int j = 0; j < LY; ++j) { a0[j] = make_float2(0.f, 0.f); a1[j] = make_float2(0.f, 0.f); }
+#pragma unroll
+                for (int i = 0; i < LY + 2 * K; ++i) {
+                    const float4 f = xp[i * (XP / 4)];
+                    const float2 lo = make_float2(f.x, f.y), hi = make_float2(f.z, f.w);
+#pragma unroll
+                    for (int j = 0; j < LY; ++j) {
+                        const int k = i - j;          // input row i contributes to output row j with tap k
+                        if (k >= 0 && k < W) {
+                            const float2 w2 = make_float2(gw.w[k], gw.w[k]);
+                            a0[j] = ffma2(w2, lo, a0[j]);
+                            a1[j] = ffma2(w2, hi, a1[j]);
+                        }
+                    }
+                }
+                const int gx = px0 + cg * 4;
+                if (gx < nx) {
+                    float* op = rout + cc * N + ((size_t)pz * ny + (py0 + h * LY)) * nx + gx;
+#pragma unroll
+                    for (int j = 0; j < LY; ++j)
+                        if (py0 + h * LY + j < ny)
+                            *reinterpret_cast<float4*>(op + (size_t)j * nx) = make_float4(a0[j].x, a0[j].y, a1[j].x, a1[j].y);
+                }
+            }
         }
+        if (!have) break;
+        __syncthreads();
+
+        // ---- phase 2 of tile t: x pass, lanes <-> rows; output x0 + g*LX + j reads U columns OFF + g*LX + j + k
+        for (int tk = tid; tk < C::P2_TASKS; tk += NT) {
+            const int r = tk % PY, q = tk / PY, g = q % (TX / LX), cc = q / (TX / LX);
+            const float4* up = reinterpret_cast<const float4*>(U + (cc * PY + r) * UP + g * LX);
+            float v[4 * NV];
+#pragma unroll
+            for (int i = 0; i < NV; ++i) {
+                const float4 f = up[i];
+                v[4 * i] = f.x; v[4 * i + 1] = f.y; v[4 * i + 2] = f.z; v[4 * i + 3] = f.w;
+            }
+            float o[LX];
+#pragma unroll
+            for (int j = 0; j < LX; ++j) {
+                float acc = 0.f;
+#pragma unroll
+                for (int k = 0; k < W; ++k) acc = fmaf(gw.w[k], v[OFF + j + k], acc);
+                o[j] = acc;
+            }
+            float4* xp = reinterpret_cast<float4*>(X + (cc * PY + r) * XP + g * LX);
+            xp[0] = make_float4(o[0], o[1], o[2], o[3]);
+            xp[1] = make_float4(o[4], o[5], o[6], o[7]);
+        }
+        __syncthreads();
+        px0 = x0; py0 = y0; pz = z; have_prev = true;
     }
 }
 
