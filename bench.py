@@ -51,7 +51,7 @@ def measured_peak_gbs():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs"""
+    """nvidia-smi clocks / throttle reasons sampled every 50 ms while the timed region runs"""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -62,7 +62,7 @@ class ClockSampler:
     def start(self):
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                       "--format=csv,noheader,nounits", "-lms", "50"],
                                       stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except OSError:
             self.p = None
@@ -139,17 +139,85 @@ def run_reference(args):
     return 0
 
 
+SWEEP_SIZES = ((64, 64, 64), (128, 128, 128), (256, 256, 256), (512, 512, 256))
+
+
+def run_sweep(args):
+    """--sweep: BASELINE.json configs[4] -- every exported kernel alone, on seeded smooth random volumes / fields, at
+    64^3 .. 512x512x256; achieved GB/s = algorithmic bytes / CUDA-event time, vs the HBM peak.
+    The working sets at 64^3 and 128^3 (and most of 256^3) fit the 126 MB L2: those rows are L2-resident numbers."""
+    import torch
+
+    import paper_1204_6295_b200 as disc
+    import phantoms
+
+    torch.cuda.set_device(0)
+    peak, peak_src = measured_peak_gbs()
+    stream = torch.cuda.current_stream()
+    rows = []
+
+    def timed(fn, n_warm=5, n=30):
+        for _ in range(n_warm):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(n):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    sizes = SWEEP_SIZES[:args.sweep_max] if args.sweep_max else SWEEP_SIZES
+    for dims in sizes:
+        nx, ny, nz = dims
+        n = nx * ny * nz
+        a, b, u = phantoms.make_sweep_inputs(dims)
+        d_a, d_b, d_u = torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda(), torch.from_numpy(u).cuda()
+        d_o, d_o2 = torch.empty_like(d_a), torch.empty_like(d_a)
+        d_r = d_u.clone()
+        tag = f"{nx}x{ny}x{nz}"
+
+        def add(kernel, param, bpv, ms):
+            gbs = bpv * n / (ms * 1e-3) / 1e9
+            rows.append({"kernel": kernel, "size": tag, "param": param, "ms": ms, "bytes_per_voxel": bpv, "gbs": gbs,
+                         "frac": gbs / peak})
+
+        ctx = disc.disc_create(dims, (1.0, 1.0, 1.0), 1, 1.0, 1, 1)
+        add("disc_warp", None, 20.0, timed(lambda: disc.disc_warp(ctx, 0, d_a, d_u, d_o)))
+        add("disc_force_update", None, 32.0, timed(lambda: disc.disc_force_update(ctx, 0, d_a, d_b, d_r)))
+        disc.disc_destroy(ctx)
+        for R in range(1, 11):
+            ctx = disc.disc_create(dims, (1.0, 1.0, 1.0), R, 1.0, 1, 1)
+            add("disc_box_moments", f"R={R}", 12.0, timed(lambda: disc.disc_box_moments(ctx, 0, d_a, d_o, d_o2)))
+            disc.disc_destroy(ctx)
+        for sigma in (1.0, 1.5, 2.0, 2.5, 3.0):
+            ctx = disc.disc_create(dims, (1.0, 1.0, 1.0), 1, sigma, 1, 1)
+            d_r.copy_(d_u)
+            add("disc_smooth_field", f"sigma={sigma}", 24.0, timed(lambda: disc.disc_smooth_field(ctx, 0, d_r)))
+            disc.disc_destroy(ctx)
+        del d_a, d_b, d_u, d_o, d_o2, d_r
+        torch.cuda.empty_cache()
+    print(json.dumps({"sweep": "config5 per-kernel", "peak_gbs": peak, "peak_source": peak_src, "unit": "GB/s",
+                      "note": "64^3 and 128^3 working sets are L2-resident; 30 back-to-back launches per point", "rows": rows}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="disc", choices=["disc", "reference"])
     ap.add_argument("--config", type=int, default=WORKLOAD_CONFIG, help="BASELINE.json config (bench line: 3)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="BASELINE.json config 5: per-kernel GB/s sweep (1 GPU)")
+    ap.add_argument("--sweep-max", type=int, default=0, help="only the first n sizes of the sweep")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
 
     import numpy as np
     import torch
@@ -182,12 +250,10 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    from paper_1204_6295_b200 import replicas
+
     def max_over_ranks(ms):
-        if dist is None:
-            return ms
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return replicas.max_over_ranks(ms, dist, "cuda")
 
     # ---------------- device-resident: K whole registrations
     for _ in range(args.warmup):

@@ -2,7 +2,7 @@
 //
 // Steps (c) and (d) of an iteration plus the warp (b) that opens the next one:
 //   k_force_gxy<K, FORCE> : [r += force(m, s')]  then the x and y Gaussian passes   -> scratch field
-//   k_gz_warp<K, WARP>    : the z Gaussian pass of the scratch field -> r, [then m = ct(x + r(x))]
+//   (the z Gaussian pass of the scratch field -> r, [then m = ct(x + r(x))] lives in field_v3.cuh)
 // Fusing the force into the x/y passes and the warp into the z pass removes one read of r (12 B/voxel)
 // and one read + one write of the un-smoothed field per iteration; the stand-alone variants
 // (FORCE = false, WARP = false) serve disc_smooth_field.
@@ -122,51 +122,6 @@ k_force_gxy(const float* __restrict__ m, const float* __restrict__ s, const floa
                     rout[c * N + o] = acc;
                 }
             }
-        }
-    }
-}
-
-// Gaussian z pass (+ warp of the moving image by the finished field).  Threads <-> (x,y) columns.
-template <int K, bool WARP>
-__global__ void __launch_bounds__(128)
-k_gz_warp(const float* __restrict__ rin, float* __restrict__ rout, const float* __restrict__ moving,
-          float* __restrict__ mout, int nx, int ny, int nz, int zchunk, GaussTaps gw) {
-    constexpr int W = 2 * K + 1;
-    const size_t plane = (size_t)nx * ny;
-    const size_t col = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (col >= plane) return;
-    const size_t N = plane * nz;
-    const int z0 = blockIdx.y * zchunk, z1 = min(z0 + zchunk, nz);
-    const int y = (int)(col / nx), x = (int)(col - (size_t)y * nx);
-
-    float ring[3][W];
-    // slices z0-K .. z0+K-1 into slots 0 .. 2K-1
-#pragma unroll
-    for (int j = 0; j < W - 1; ++j) {
-        const size_t o = (size_t)clampi(z0 - K + j, 0, nz - 1) * plane + col;
-#pragma unroll
-        for (int c = 0; c < 3; ++c) ring[c][j] = __ldg(rin + c * N + o);
-    }
-    for (int zb = z0; zb < z1; zb += W) {
-#pragma unroll
-        for (int j = 0; j < W; ++j) {
-            const int z = zb + j;
-            if (z >= z1) break;
-            const size_t oin = (size_t)clampi(z + K, 0, nz - 1) * plane + col;  // replicate border in z
-#pragma unroll
-            for (int c = 0; c < 3; ++c) ring[c][(j + W - 1) % W] = __ldg(rin + c * N + oin);
-            float r[3];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                float acc = 0.f;
-#pragma unroll
-                for (int k = 0; k < W; ++k) acc = fmaf(gw.w[k], ring[c][(j + k) % W], acc);
-                r[c] = acc;
-            }
-            const size_t o = (size_t)z * plane + col;
-            rout[o] = r[0]; rout[N + o] = r[1]; rout[2 * N + o] = r[2];
-            if (WARP)
-                mout[o] = trilinear_clamped(moving, nx, ny, nz, (float)x + r[0], (float)y + r[1], (float)z + r[2]);
         }
     }
 }

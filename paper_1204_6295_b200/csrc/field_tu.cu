@@ -1,9 +1,8 @@
-// field_tu.cu -- instantiates k_force_gxy<K,...> and k_gz_warp<K,...> for K in [DISC_K_LO, DISC_K_HI]; built
+// field_tu.cu -- instantiates the force+Gxy and Gz+warp kernels (field.cuh, field_v3.cuh) for K in [DISC_K_LO, DISC_K_HI]; built
 // once per range (-DDISC_TU=n -DDISC_K_LO=a -DDISC_K_HI=b).  TU 0 also holds the K-independent kernels.
 #include <cstdlib>
 
 #include "field.cuh"
-#include "field_v2.cuh"
 #include "field_v3.cuh"
 #include "launch.h"
 

@@ -1,20 +1,76 @@
-// field_v3.cuh -- third generation of the two field kernels (same arithmetic as field.cuh, same results up to
-// fp32 rounding order).  profiles/r01b showed both second-generation kernels bound by their INSTRUCTION COUNT
-// (280-290 thread instructions per voxel, a quarter of them pipeline bookkeeping and 64-bit address arithmetic)
-// and by the exposed latency of their loads.  Here:
+// field_v3.cuh -- the two field kernels of the iteration (same arithmetic as the plain kernels of field.cuh, same
+// results up to fp32 rounding order):
+//   k_force_gxy_t4<K, FORCE>      [r += force(m, s')], Gaussian x pass, Gaussian y pass -> scratch field
+//   k_gz_warp_d / _d2<K, WARP, LZ> Gaussian z pass of the scratch field -> r, [then m = ct(x + r(x))]
 //
-//   k_gz_warp_d<K, WARP, LZ>   Gaussian z pass (+ warp).  No ring, no shared memory, no barriers: a thread owns ONE
-//                              (x,y) column and LZ consecutive output slices; per component it issues all LZ + 2K
-//                              input loads at once (coalesced across the warp, latency overlapped LZ + 2K deep),
-//                              forms the LZ outputs with statically indexed registers, and then runs the warp's
-//                              trilinear gathers in batches of four voxels (32 independent loads in flight).
-//                              The input is re-read (LZ + 2K)/LZ times, but only from L2: neighbouring z blocks
-//                              run at the same time on other SMs.
+// History (profiles/r01a, r01b): the marching ring kernels of the first two generations were bound by their
+// INSTRUCTION COUNT (280-290 thread instructions per voxel, a quarter of them pipeline bookkeeping and 64-bit
+// address arithmetic) and by the exposed latency of their loads, not by HBM.  Hence
+//   * z pass + warp: no ring, no shared memory, no barriers.  A thread owns one (or two adjacent) (x,y) columns
+//     and LZ consecutive output slices; per component it issues all LZ + 2K input loads at once (coalesced
+//     across the warp, latency overlapped LZ + 2K deep), forms the LZ outputs from statically indexed registers,
+//     then runs the warp's trilinear gathers in batches (16-32 independent loads in flight).  The input is
+//     re-read (LZ + 2K)/LZ times, but only from L2: neighbouring z blocks run at the same time on other SMs.
+//   * force + x + y passes: a persistent tile kernel whose phase 1 works on groups of four x-adjacent points
+//     with 16-byte loads (see below).
 #pragma once
 #include "common.cuh"
-#include "field_v2.cuh"
+#include "field.cuh"
+#include "pipeline.cuh"
 
 namespace disc {
+
+// The eight neighbours and three weights of one trilinear sample (reading A11), split in two halves so that the
+// loads can be issued long before they are used.
+struct TriSample {
+    float a[8];
+    float tx, ty, tz;
+};
+
+// FAST: every axis has at least two voxels (checked once per kernel, uniform), so the neighbour offsets are the
+// constants +1, +nx, +plane and the eight addresses share four row pointers.
+template <bool FAST>
+__device__ __forceinline__ void tri_issue(const float* __restrict__ I, int nx, int ny, int nz, float px, float py,
+                                          float pz, TriSample& s) {
+    px = fminf(fmaxf(px, 0.f), (float)(nx - 1));
+    py = fminf(fmaxf(py, 0.f), (float)(ny - 1));
+    pz = fminf(fmaxf(pz, 0.f), (float)(nz - 1));
+    if (FAST) {
+        const int x0 = min((int)px, nx - 2), y0 = min((int)py, ny - 2), z0 = min((int)pz, nz - 2);
+        s.tx = px - (float)x0; s.ty = py - (float)y0; s.tz = pz - (float)z0;
+        const float* p00 = I + ((size_t)(unsigned)((z0 * ny + y0) * nx + x0));
+        const float* p10 = p00 + nx;
+        const float* p01 = p00 + (size_t)nx * ny;
+        const float* p11 = p01 + nx;
+        s.a[0] = __ldg(p00); s.a[1] = __ldg(p00 + 1);
+        s.a[2] = __ldg(p10); s.a[3] = __ldg(p10 + 1);
+        s.a[4] = __ldg(p01); s.a[5] = __ldg(p01 + 1);
+        s.a[6] = __ldg(p11); s.a[7] = __ldg(p11 + 1);
+    } else {
+        const int x0 = max(min((int)px, nx - 2), 0), y0 = max(min((int)py, ny - 2), 0), z0 = max(min((int)pz, nz - 2), 0);
+        const int dx = nx > 1 ? 1 : 0;
+        const int dy = ny > 1 ? nx : 0;
+        const size_t dz = nz > 1 ? (size_t)nx * ny : 0;
+        s.tx = px - (float)x0; s.ty = py - (float)y0; s.tz = pz - (float)z0;
+        const float* p = I + ((size_t)z0 * ny + y0) * nx + x0;
+        s.a[0] = __ldg(p); s.a[1] = __ldg(p + dx);
+        s.a[2] = __ldg(p + dy); s.a[3] = __ldg(p + dy + dx);
+        s.a[4] = __ldg(p + dz); s.a[5] = __ldg(p + dz + dx);
+        s.a[6] = __ldg(p + dz + dy); s.a[7] = __ldg(p + dz + dy + dx);
+    }
+}
+
+__device__ __forceinline__ float tri_finish(const TriSample& s) {
+    // (1-t)*a + t*b: exact at t = 0 and t = 1, so a zero field reproduces the input bit for bit
+    const float ux = 1.f - s.tx, uy = 1.f - s.ty, uz = 1.f - s.tz;
+    const float c00 = fmaf(s.tx, s.a[1], ux * s.a[0]);
+    const float c10 = fmaf(s.tx, s.a[3], ux * s.a[2]);
+    const float c01 = fmaf(s.tx, s.a[5], ux * s.a[4]);
+    const float c11 = fmaf(s.tx, s.a[7], ux * s.a[6]);
+    const float c0 = fmaf(s.ty, c10, uy * c00);
+    const float c1 = fmaf(s.ty, c11, uy * c01);
+    return fmaf(s.tz, c1, uz * c0);
+}
 
 constexpr int kGzdThreads = 128;
 
