@@ -112,7 +112,7 @@ void pick_moments_shape(const disc_ctx* c, const Level& L, int* ty_out, int* zch
             const int zc = (L.nz + nchunk - 1) / nchunk;
             const long long ctas = tiles * ((L.nz + zc - 1) / zc);
             const long long waves = (ctas + slots - 1) / slots;
-            const double cost = (double)waves * (zc + 2 * R + 6) * (ty + R + 4) * (ty == 16 ? 1.6 : 1.0);
+            const double cost = (double)waves * (zc + 2 * R + 6) * (ty + R + 4) * (ty == 16 ? 1.8 : 1.0);
             if (cost < best) { best = cost; best_ty = ty; best_zc = zc; }
             if (zc == 1) break;
         }

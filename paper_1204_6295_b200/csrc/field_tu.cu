@@ -16,18 +16,19 @@ static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t
 template <int K, bool FORCE>
 static void launch_fg(int txb, const float* m, const float* s, const float* rin, float* rout, int nx, int ny, int nz,
                       int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
-    if (nx % 4 == 0 && aligned16(rin) && aligned16(rout) && (!FORCE || (aligned16(m) && aligned16(s)))) {
+    const bool vec_ok = nx % 4 == 0 && aligned16(rin) && aligned16(rout) && (!FORCE || (aligned16(m) && aligned16(s)));
+    static int n_sm = 0;
+    if (!n_sm) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    }
+    if (vec_ok) {
         using C = FgT4Cfg<K>;
         static bool configured = false;  // one attribute call per instance (idempotent, so a race is harmless)
         if (!configured) {
             cudaFuncSetAttribute(k_force_gxy_t4<K, FORCE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
             configured = true;
-        }
-        static int n_sm = 0;
-        if (!n_sm) {
-            int dev = 0;
-            cudaGetDevice(&dev);
-            cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
         }
         const long long n_tiles = (long long)((nx + C::TX - 1) / C::TX) * ((ny + C::TY - 1) / C::TY) * nz;
         const int grid = (int)(n_tiles < (long long)C::OCC * n_sm ? n_tiles : (long long)C::OCC * n_sm);   // persistent: OCC CTAs per SM

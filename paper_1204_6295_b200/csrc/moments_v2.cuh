@@ -44,7 +44,12 @@ struct MomV2Cfg {
     // an odd number of 16-byte chunks (lanes <-> rows reads are then bank-conflict free).
     static constexpr int RA = (R + 3) / 4 * 4, OFF = RA - R;
     static constexpr int PXB = (((OFF + PX + 3) / 4) | 1) * 4;
-    static constexpr int NSTG = 8, NXS = 3, NAUX = 8;                  // raw stages, exchange buffers, aux stages
+#ifndef DISC_MOM_NSTG
+#define DISC_MOM_NSTG 8
+#define DISC_MOM_NXS 3
+#define DISC_MOM_NAUX 8
+#endif
+    static constexpr int NSTG = DISC_MOM_NSTG, NXS = DISC_MOM_NXS, NAUX = DISC_MOM_NAUX;                  // raw stages, exchange buffers, aux stages
     static constexpr int XSP = TX + 1;                                 // exchange-row pitch in (S1,S2) pairs, odd
     static constexpr size_t raw_bytes = sizeof(float) * PY * PXB;      // one stage; multiple of 16
     static constexpr size_t raw_stride = (raw_bytes + 127) / 128 * 128;
