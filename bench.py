@@ -322,11 +322,14 @@ def main():
         gbs = bpv * n0 / (ms * 1e-3) / 1e9
         per_kernel.append({"kernel": name, "ms": ms, "bytes_per_voxel": bpv, "gbs": gbs, "frac": gbs / peak})
     dom = max(per_kernel, key=lambda k: k["ms"])
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")     # written from an `ncu --set full` capture, per launch
+    traffic = None                                              # dram bytes per launch from the latest `ncu --set full`
+    tpath = os.path.join(ROOT, "profiles", "r01c_traffic.csv")  # capture (profiles/r01c_launches_and_ncu.md), text only
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get(dom["kernel"])
+            for ln in open(tpath).read().splitlines()[1:]:
+                f = ln.split(",")
+                if f[0] == dom["kernel"]:
+                    traffic = float(f[1])
         except Exception:
             traffic = None
     roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["gbs"], "peak": peak, "unit": "GB/s",
