@@ -126,13 +126,15 @@ def correct_at(cbct, ct_warped, R, idx, eps_var=EPS_VAR):
     return out
 
 
-def force_update(m, s, disp, eps_den=EPS_DEN):
-    """r += (s'-m) grad s' / (|grad s'|^2 + (s'-m)^2 + eps) (PAPER.md:73 Eq. 1 first term, :192-193; readings A1, A7, A8)."""
+def force_update(m, s, disp, eps_den=EPS_DEN, double_force=False):
+    """r += (s'-m) grad s' / (|grad s'|^2 + (s'-m)^2 + eps) (PAPER.md:73 Eq. 1 first term, :192-193; readings A1, A7, A8);
+    with double_force also the second term of Eq. 1, + (s'-m) grad m / (|grad m|^2 + (s'-m)^2 + eps)."""
     L = _load()
     m_, pm = _f32(m)
     s_, ps = _f32(s)
     d = np.array(disp, dtype=np.float32, order="C", copy=True)
-    L.oracle_force_update(pm, ps, *_dims(m_), ctypes.c_double(eps_den), d.ctypes.data_as(_f32p))
+    fn = L.oracle_force_update_double if double_force else L.oracle_force_update
+    fn(pm, ps, *_dims(m_), ctypes.c_double(eps_den), d.ctypes.data_as(_f32p))
     return d
 
 
@@ -172,12 +174,13 @@ def upsample_field(disp):
     return out
 
 
-def demons_step(m, s, disp, sigma, eps_den=EPS_DEN):
+def demons_step(m, s, disp, sigma, eps_den=EPS_DEN, double_force=False):
     """Alg. A1 steps 4-6."""
-    return smooth_field(force_update(m, s, disp, eps_den), sigma)
+    return smooth_field(force_update(m, s, disp, eps_den, double_force), sigma)
 
 
-def register(ct, cbct, R, sigma, levels, iters, eps_var=EPS_VAR, eps_den=EPS_DEN, want_corr=True, want_trace=False):
+def register(ct, cbct, R, sigma, levels, iters, eps_var=EPS_VAR, eps_den=EPS_DEN, want_corr=True, want_trace=False,
+             double_force=False):
     """Algorithm A1 with a fixed iteration count (readings A9, A12, A14)."""
     L = _load()
     a, pa = _f32(ct)
@@ -185,9 +188,9 @@ def register(ct, cbct, R, sigma, levels, iters, eps_var=EPS_VAR, eps_den=EPS_DEN
     disp = np.empty((3,) + a.shape, dtype=np.float32)
     corr = np.empty_like(a) if want_corr else None
     trace = np.zeros(levels * iters, dtype=np.float64) if want_trace else None
-    L.oracle_register(pa, pb, *_dims(a), ctypes.c_int(R), ctypes.c_double(sigma), ctypes.c_int(levels),
-                      ctypes.c_int(iters), ctypes.c_double(eps_var), ctypes.c_double(eps_den),
-                      disp.ctypes.data_as(_f32p), corr.ctypes.data_as(_f32p) if want_corr else None,
+    L.oracle_register_mode(pa, pb, *_dims(a), ctypes.c_int(R), ctypes.c_double(sigma), ctypes.c_int(levels),
+                           ctypes.c_int(iters), ctypes.c_double(eps_var), ctypes.c_double(eps_den),
+                           ctypes.c_int(1 if double_force else 0), disp.ctypes.data_as(_f32p), corr.ctypes.data_as(_f32p) if want_corr else None,
                       trace.ctypes.data_as(_f64p) if want_trace else None)
     out = (disp, corr)
     return out + (trace,) if want_trace else out

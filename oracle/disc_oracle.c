@@ -191,6 +191,33 @@ void oracle_force_update(const float *m, const float *s, int nx, int ny, int nz,
             }
 }
 
+/* NEXT-2: the double-force variant, both terms of Eq. (1): the passive force with the gradient
+ * of the (corrected) static image plus the active force with the gradient of the deformed moving image I_m^(k),
+ * each with its own denominator.  Same sign convention (reading A1), same central differences with clamped
+ * indices (A8) and the same eps_den in both denominators (A7):
+ *   d = s' - m,  r_c += d g_c / (|g|^2 + d^2 + eps) + d h_c / (|h|^2 + d^2 + eps),  g = grad s', h = grad m. */
+void oracle_force_update_double(const float *m, const float *s, int nx, int ny, int nz, double eps_den, float *disp) {
+    size_t N = (size_t)nx * ny * nz;
+#pragma omp parallel for schedule(static)
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) {
+                size_t i = IDX(x, y, z);
+                size_t xp = IDX(clampi(x + 1, 0, nx - 1), y, z), xm = IDX(clampi(x - 1, 0, nx - 1), y, z);
+                size_t yp = IDX(x, clampi(y + 1, 0, ny - 1), z), ym = IDX(x, clampi(y - 1, 0, ny - 1), z);
+                size_t zp = IDX(x, y, clampi(z + 1, 0, nz - 1)), zm = IDX(x, y, clampi(z - 1, 0, nz - 1));
+                double g[3] = {0.5 * ((double)s[xp] - (double)s[xm]), 0.5 * ((double)s[yp] - (double)s[ym]),
+                               0.5 * ((double)s[zp] - (double)s[zm])};
+                double h[3] = {0.5 * ((double)m[xp] - (double)m[xm]), 0.5 * ((double)m[yp] - (double)m[ym]),
+                               0.5 * ((double)m[zp] - (double)m[zm])};
+                double d = (double)s[i] - (double)m[i];
+                double den_s = g[0] * g[0] + g[1] * g[1] + g[2] * g[2] + d * d + eps_den;
+                double den_m = h[0] * h[0] + h[1] * h[1] + h[2] * h[2] + d * d + eps_den;
+                for (int c = 0; c < 3; ++c)
+                    disp[c * N + i] = (float)((double)disp[c * N + i] + d * g[c] / den_s + d * h[c] / den_m);
+            }
+}
+
 /* ------------------------------------------------------------------------
  * (d) Gaussian regularisation of the total field r (Alg. A1 step 6,
  * PAPER.md:194).  Reading A10: K = ceil(3 sigma), w_i ~ exp(-i^2 / 2 sigma^2)
@@ -283,8 +310,9 @@ void oracle_upsample_field(const float *dc, int cx, int cy, int cz, float *out) 
  * they are computed once per level with the same naive loop.
  * `trace` (optional, may be NULL): receives sum|r| after every iteration.
  * ---------------------------------------------------------------------- */
-void oracle_register(const float *ct, const float *cbct, int nx, int ny, int nz, int R, double sigma, int levels,
-                     int iters, double eps_var, double eps_den, float *out_disp, float *out_corr, double *trace) {
+void oracle_register_mode(const float *ct, const float *cbct, int nx, int ny, int nz, int R, double sigma, int levels,
+                          int iters, double eps_var, double eps_den, int double_force, float *out_disp,
+                          float *out_corr, double *trace) {
     const float **pct = (const float **)malloc(sizeof(float *) * levels);
     const float **pcb = (const float **)malloc(sizeof(float *) * levels);
     pct[0] = ct; pcb[0] = cbct;
@@ -316,7 +344,8 @@ void oracle_register(const float *ct, const float *cbct, int nx, int ny, int nz,
             oracle_warp(pct[l], r, lx, ly, lz, m);                                   /* I_m^(k) */
             oracle_box_moments(m, lx, ly, lz, R, mum, vm);                           /* A1 step 1 */
             oracle_correct_from_moments(pcb[l], mus, vs, mum, vm, N, eps_var, sp);   /* A1 step 3 */
-            oracle_force_update(m, sp, lx, ly, lz, eps_den, r);                      /* A1 steps 4-5 */
+            if (double_force) oracle_force_update_double(m, sp, lx, ly, lz, eps_den, r); /* Eq. (1), both terms */
+            else oracle_force_update(m, sp, lx, ly, lz, eps_den, r);                 /* A1 steps 4-5 */
             oracle_smooth_field(r, lx, ly, lz, sigma);                               /* A1 step 6 */
             if (trace) {
                 double s = 0.0;
@@ -338,4 +367,10 @@ void oracle_register(const float *ct, const float *cbct, int nx, int ny, int nz,
     free(r);
     for (int l = 1; l < levels; ++l) { free((void *)pct[l]); free((void *)pcb[l]); }
     free(pct); free(pcb);
+}
+
+/* north_star's schedule: the Thirion (single, passive) force */
+void oracle_register(const float *ct, const float *cbct, int nx, int ny, int nz, int R, double sigma, int levels,
+                     int iters, double eps_var, double eps_den, float *out_disp, float *out_corr, double *trace) {
+    oracle_register_mode(ct, cbct, nx, ny, nz, R, sigma, levels, iters, eps_var, eps_den, 0, out_disp, out_corr, trace);
 }

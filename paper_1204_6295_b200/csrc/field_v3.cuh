@@ -190,7 +190,10 @@ k_gz_warp_d2(const float* __restrict__ rin, float* __restrict__ rout, const floa
         const float fx0 = (float)x, fx1 = (float)(x + 1), fy = (float)y;
         const bool fast = nx > 1 && ny > 1 && nz > 1 && N < (size_t)0x7fffffff;   // 32-bit voxel indices
         float* mp = mout + (size_t)z0 * plane + col;
-        constexpr int B = 2;
+#ifndef DISC_GZ_B
+#define DISC_GZ_B 1
+#endif
+        constexpr int B = DISC_GZ_B;
         static_assert(LZ % B == 0, "gather batches");
 #pragma unroll
         for (int j0 = 0; j0 < LZ; j0 += B) {

@@ -196,6 +196,56 @@ def test_P10_force(oracle_mod):
     np.testing.assert_allclose(d[0, :, :, 0], dd * gb / (gb * gb + dd * dd), rtol=1e-6)
 
 
+def test_double_force_pins(oracle_mod):
+    """NEXT-2, both terms of Eq. (1): closed forms and symmetries, none re-typing the formula."""
+    rng = np.random.default_rng(12)
+    shape = (6, 7, 8)
+    s = rng.normal(0, 100, size=shape).astype(np.float32)
+    m = rng.normal(0, 100, size=shape).astype(np.float32)
+    r0 = rng.normal(0, 1, size=(3,) + shape).astype(np.float32)
+    zero = np.zeros_like(r0)
+    f2 = lambda mm, ss, r, **kw: oracle_mod.force_update(mm, ss, r, double_force=True, **kw)
+    assert np.array_equal(f2(s, s, r0), r0)                                            # m = s' -> dr = 0
+    # a flat moving image has no active force: the double force reduces to the Thirion force ...
+    flat = np.full(shape, 5.0, dtype=np.float32)
+    assert np.array_equal(f2(flat, s, zero), oracle_mod.force_update(flat, s, zero))
+    # ... and a flat static image leaves ONLY the active term = the Thirion force with the roles swapped, negated
+    np.testing.assert_allclose(f2(m, flat, zero), -oracle_mod.force_update(flat, m, zero), rtol=1e-6, atol=1e-7)
+    # exchanging the two images negates the double force exactly (each term maps onto the other)
+    assert np.array_equal(f2(m, s, zero), -f2(s, m, zero))
+    # each term is bounded by 1/2 (AM-GM) -> |dr| <= 1
+    d = f2(m, s, zero)
+    assert np.sqrt((d.astype(np.float64) ** 2).sum(0)).max() <= 1.0 + 1e-6
+    # ramp: s' = g x, m = s' - g delta: both gradients equal g -> twice the single force, 2 delta / (1 + delta^2)
+    z, y, x = np.meshgrid(np.arange(6.), np.arange(7.), np.arange(8.), indexing="ij")
+    for g, delta in ((10.0, 0.5), (200.0, 2.0), (-30.0, 0.25)):
+        sp = (g * x).astype(np.float32)
+        mm = (g * x - g * delta).astype(np.float32)
+        d = f2(mm, sp, zero, eps_den=0.0)[:, :, :, 1:-1]
+        np.testing.assert_allclose(d[0], 2 * delta / (1 + delta ** 2), rtol=1e-6)
+        assert np.all(d[1] == 0) and np.all(d[2] == 0)
+    # different slopes: s' = g x, m = h x - c  ->  d g/(g^2+d^2) + d h/(h^2+d^2) with d = s' - m evaluated per voxel
+    g, h, c = 12.0, 7.0, 3.0
+    sp, mm = (g * x).astype(np.float32), (h * x - c).astype(np.float32)
+    dd = (g - h) * x[:, :, 1:-1] + c
+    want = dd * g / (g * g + dd * dd) + dd * h / (h * h + dd * dd)
+    np.testing.assert_allclose(f2(mm, sp, zero, eps_den=0.0)[0, :, :, 1:-1], want, rtol=1e-6)
+
+
+def test_double_force_recovers_a_translation(oracle_mod):
+    """whole loop with the double force: same sign convention as P11, converges at least as far as the single force"""
+    ct, _, _, _ = phantoms.make_pair(1, dims=(48, 40, 24))
+    u = np.zeros((3,) + ct.shape, dtype=np.float32); u[0], u[1], u[2] = 2.0, -1.0, 1.0
+    target = phantoms.pullback(ct, u)
+    rng = np.random.default_rng(5)
+    cbct = (0.9 * target + rng.normal(0, 20, ct.shape)).astype(np.float32)
+    rmse = lambda r: float(np.sqrt(np.mean((oracle_mod.warp(ct, r) - target) ** 2)))
+    r1, _ = oracle_mod.register(ct, cbct, 3, 1.5, 1, 40, want_corr=False)
+    r2, _ = oracle_mod.register(ct, cbct, 3, 1.5, 1, 40, want_corr=False, double_force=True)
+    e0, e1, e2 = rmse(np.zeros_like(u)), rmse(r1), rmse(r2)
+    assert e2 < e0 / 2.5 and e2 < 1.1 * e1, (e0, e1, e2)
+
+
 def test_force_components_and_axes(oracle_mod):
     """each component uses its own axis' gradient (catches transposed strides)."""
     z, y, x = np.meshgrid(np.arange(5.), np.arange(6.), np.arange(7.), indexing="ij")
