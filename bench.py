@@ -288,6 +288,16 @@ def main():
     f1.record(stream)
     torch.cuda.synchronize()
     ms_iter = f0.elapsed_time(f1) / 100.0          # includes the per-call z-score + warp prologue (2 of 302 launches)
+    # the paper's double-force variant (both terms of Eq. 1): same loop, reported beside the headline
+    disc.disc_set_force(ctx, disc.DISC_FORCE_DOUBLE)
+    disc.disc_iterate(ctx, 0, d_ct, d_cb, d_r2, 5)
+    torch.cuda.synchronize()
+    f0.record(stream)
+    disc.disc_iterate(ctx, 0, d_ct, d_cb, d_r2, 100)
+    f1.record(stream)
+    torch.cuda.synchronize()
+    ms_iter_double = f0.elapsed_time(f1) / 100.0
+    disc.disc_set_force(ctx, disc.DISC_FORCE_THIRION)
     clocks = sampler.stop() if rank == 0 else None
 
     # ---------------- end to end: pinned host buffers through disc_register_host
@@ -352,6 +362,7 @@ def main():
                    "l2": "working set 320 MiB > 126 MB L2 (inputs larger than L2)"},
         "iterations_per_s_finest": 1e3 / ms_iter, "voxel_updates_per_s_finest": n0 * 1e3 / ms_iter,
         "ms_per_iteration_finest": ms_iter,
+        "double_force": {"ms_per_iteration_finest": ms_iter_double, "iterations_per_s_finest": 1e3 / ms_iter_double},
         "e2e": {"value": e2e_value, "unit": "voxel-updates/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": ms_e2e / n_e2e},
         "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,

@@ -78,6 +78,18 @@ const char* disc_last_error(const disc_ctx* ctx);
 /* Number of CUDA kernels this context has launched so far (bench.py's gpu_launches). */
 unsigned long long disc_launch_count(const disc_ctx* ctx);
 
+/* Force variant used by disc_force_update, disc_demons_step, disc_iterate and disc_register from now on.
+ *   DISC_FORCE_THIRION (default): the passive force, first term of Eq. (1) with the corrected CBCT s'
+ *                      (north_star (c); reading A2):  dr = d grad(s') / (|grad s'|^2 + d^2 + eps)
+ *   DISC_FORCE_DOUBLE: both terms of Eq. (1), the paper's double-force demons:
+ *                      dr = d grad(s') / (|grad s'|^2 + d^2 + eps) + d grad(m) / (|grad m|^2 + d^2 + eps)
+ * with d = s' - m (sign: reading A1), m the deformed CT of the current iteration, both gradients central
+ * differences with clamped indices (A8), eps = DISC_EPS_DEN in both denominators (A7).
+ * Host-side state only, no launch.  Any other mode -> DISC_ERR_INVALID_ARG. */
+#define DISC_FORCE_THIRION 1
+#define DISC_FORCE_DOUBLE 2
+disc_status disc_set_force(disc_ctx* ctx, int mode);
+
 /* ---- the steps of one iteration, in execution order b -> a -> c+d (Alg. A1) ---- */
 
 /* (b) out(x) = moving(x + disp(x)), trilinear, sample position clamped to the volume

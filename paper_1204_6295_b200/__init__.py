@@ -20,9 +20,10 @@ DISC_MAX_PATCH_RADIUS = 10
 DISC_MAX_GAUSS_RADIUS = 12
 DISC_EPS_VAR = 1e-6
 DISC_EPS_DEN = 1e-3
+DISC_FORCE_THIRION, DISC_FORCE_DOUBLE = 1, 2
 
 EXPORTS = (
-    "disc_create", "disc_destroy", "disc_last_error", "disc_launch_count", "disc_warp", "disc_correct_intensity",
+    "disc_create", "disc_destroy", "disc_last_error", "disc_launch_count", "disc_set_force", "disc_warp", "disc_correct_intensity",
     "disc_demons_step", "disc_register", "disc_register_host", "disc_iterate", "disc_box_moments",
     "disc_force_update", "disc_smooth_field", "disc_downsample", "disc_upsample_field", "disc_profile_iteration",
 )
@@ -43,6 +44,8 @@ _lib.disc_last_error.restype = ctypes.c_char_p
 _lib.disc_last_error.argtypes = [_vp]
 _lib.disc_launch_count.restype = ctypes.c_ulonglong
 _lib.disc_launch_count.argtypes = [_vp]
+_lib.disc_set_force.restype = _i
+_lib.disc_set_force.argtypes = [_vp, _i]
 for _name, _nptr in (("disc_warp", 3), ("disc_correct_intensity", 3), ("disc_demons_step", 3),
                      ("disc_box_moments", 3), ("disc_force_update", 3), ("disc_smooth_field", 1),
                      ("disc_downsample", 2), ("disc_upsample_field", 2)):
@@ -150,6 +153,10 @@ def disc_last_error(ctx: Ctx | None) -> str:
 
 def disc_launch_count(ctx: Ctx) -> int:
     return int(_lib.disc_launch_count(ctx.handle))
+
+
+def disc_set_force(ctx, mode):
+    _check(ctx.handle, _lib.disc_set_force(ctx.handle, int(mode)))
 
 
 def disc_warp(ctx, level, moving, disp, out, stream=None):

@@ -39,6 +39,7 @@ struct disc_ctx {
     float sigma;
     int levels, iters;
     int K;
+    int force_mode;   // 1 Thirion (default), 2 double force
     int n_sm;
     GaussTaps taps;
     Level lv[DISC_MAX_LEVELS];
@@ -131,9 +132,10 @@ disc_status launch_moments(disc_ctx* c, const Level& L, const float* vol, const 
     return check_launch(c, "k_moments");
 }
 
-template <bool FORCE>
-disc_status launch_force_gxy(disc_ctx* c, const Level& L, const float* m, const float* s, const float* rin,
+// force: 0 = plain smoothing, otherwise the context's force mode
+disc_status launch_force_gxy(disc_ctx* c, bool force, const Level& L, const float* m, const float* s, const float* rin,
                              float* rout, cudaStream_t st) {
+    const int FORCE = force ? c->force_mode : 0;
     const int txb = L.nx > 64 ? 128 : (L.nx > 32 ? 64 : 32);
     const int xt = (L.nx + txb - 1) / txb;
     const int K = c->K;
@@ -182,7 +184,7 @@ disc_status iterate_level(disc_ctx* c, Level& L, const float* ct, float* disp, i
                           cudaStream_t st) {
     for (int k = 0; k < n_iters; ++k) {
         DISC_TRY(launch_moments<kModeCorrect>(c, L, L.m, L.zhat, L.sp, nullptr, st));       // A1 steps 1,3
-        DISC_TRY(launch_force_gxy<true>(c, L, L.m, L.sp, disp, L.scratch, st));              // A1 steps 4,5,6(x,y)
+        DISC_TRY(launch_force_gxy(c, true, L, L.m, L.sp, disp, L.scratch, st));              // A1 steps 4,5,6(x,y)
         if (k + 1 < n_iters || final_warp)
             DISC_TRY(launch_gz_warp<true>(c, L, L.scratch, disp, ct, L.m, st));              // A1 step 6(z) + next I_m^(k)
         else
@@ -242,6 +244,7 @@ disc_status disc_create(disc_ctx** out, const int dims[3], const float spacing[3
     c->n_sm = 148;
     cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
     c->R = patch_radius; c->sigma = sigma_smooth; c->levels = levels; c->iters = iters; c->K = K;
+    c->force_mode = DISC_FORCE_THIRION;
     // Gaussian taps: fp64, normalised to sum 1, then rounded to fp32 (reading A10)
     {
         double w[kMaxGaussTaps], sum = 0.0;
@@ -278,6 +281,13 @@ const char* disc_last_error(const disc_ctx* ctx) { return ctx ? ctx->err : g_cre
 
 unsigned long long disc_launch_count(const disc_ctx* ctx) { return ctx ? ctx->launches : 0ull; }
 
+disc_status disc_set_force(disc_ctx* c, int mode) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_NEED(c, mode == DISC_FORCE_THIRION || mode == DISC_FORCE_DOUBLE, "force mode must be DISC_FORCE_THIRION or DISC_FORCE_DOUBLE");
+    c->force_mode = mode;
+    return DISC_OK;
+}
+
 disc_status disc_warp(disc_ctx* c, int level, const float* moving, const float* disp, float* out, void* stream) {
     if (!c) return DISC_ERR_INVALID_ARG;
     DISC_NEED(c, level_ok(c, level), "level out of range");
@@ -303,7 +313,7 @@ disc_status disc_demons_step(disc_ctx* c, int level, const float* m_warped, cons
     DISC_NEED(c, m_warped && s_corrected && disp_inout, "NULL pointer");
     Level& L = c->lv[level];
     cudaStream_t st = (cudaStream_t)stream;
-    DISC_TRY(launch_force_gxy<true>(c, L, m_warped, s_corrected, disp_inout, L.scratch, st));
+    DISC_TRY(launch_force_gxy(c, true, L, m_warped, s_corrected, disp_inout, L.scratch, st));
     return launch_gz_warp<false>(c, L, L.scratch, disp_inout, nullptr, nullptr, st);
 }
 
@@ -338,7 +348,7 @@ disc_status disc_profile_iteration(disc_ctx* c, int level, const float* ct, cons
         cudaEventRecord(ev[4 * k + 0], st);
         rc = launch_moments<kModeCorrect>(c, L, L.m, L.zhat, L.sp, nullptr, st);
         cudaEventRecord(ev[4 * k + 1], st);
-        if (rc == DISC_OK) rc = launch_force_gxy<true>(c, L, L.m, L.sp, disp_inout, L.scratch, st);
+        if (rc == DISC_OK) rc = launch_force_gxy(c, true, L, L.m, L.sp, disp_inout, L.scratch, st);
         cudaEventRecord(ev[4 * k + 2], st);
         if (rc == DISC_OK) rc = launch_gz_warp<true>(c, L, L.scratch, disp_inout, ct, L.m, st);
         cudaEventRecord(ev[4 * k + 3], st);
@@ -430,7 +440,7 @@ disc_status disc_force_update(disc_ctx* c, int level, const float* m, const floa
     DISC_NEED(c, level_ok(c, level), "level out of range");
     DISC_NEED(c, m && s && disp_inout, "NULL pointer");
     const Level& L = c->lv[level];
-    launch_force_update(m, s, disp_inout, L.nx, L.ny, L.nz, DISC_EPS_DEN, (cudaStream_t)stream);
+    launch_force_update(c->force_mode, m, s, disp_inout, L.nx, L.ny, L.nz, DISC_EPS_DEN, (cudaStream_t)stream);
     return check_launch(c, "k_force_update");
 }
 
@@ -440,7 +450,7 @@ disc_status disc_smooth_field(disc_ctx* c, int level, float* disp_inout, void* s
     DISC_NEED(c, disp_inout, "NULL pointer");
     Level& L = c->lv[level];
     cudaStream_t st = (cudaStream_t)stream;
-    DISC_TRY(launch_force_gxy<false>(c, L, nullptr, nullptr, disp_inout, L.scratch, st));
+    DISC_TRY(launch_force_gxy(c, false, L, nullptr, nullptr, disp_inout, L.scratch, st));
     return launch_gz_warp<false>(c, L, L.scratch, disp_inout, nullptr, nullptr, st);
 }
 

@@ -17,8 +17,12 @@
 
 namespace disc {
 
-// r_c(x,y,z) after the force update (or just r_c when FORCE = false); x,y,z must be in range.
-template <bool FORCE>
+// Force modes: none (plain field), the Thirion / passive force of north_star (c), and the double force = both terms
+// of Eq. (1), which adds d grad(m) / (|grad m|^2 + d^2 + eps).
+enum ForceMode { kForceNone = 0, kForceSingle = 1, kForceDouble = 2 };
+
+// r_c(x,y,z) after the force update (or just r_c when MODE = kForceNone); x,y,z must be in range.
+template <int MODE>
 __device__ __forceinline__ void updated_field(const float* __restrict__ m, const float* __restrict__ s,
                                               const float* __restrict__ rin, int nx, int ny, int nz, size_t N,
                                               int x, int y, int z, float eps_den, float out[3]) {
@@ -27,22 +31,34 @@ __device__ __forceinline__ void updated_field(const float* __restrict__ m, const
     out[0] = __ldg(rin + i);
     out[1] = __ldg(rin + N + i);
     out[2] = __ldg(rin + 2 * N + i);
-    if (FORCE) {
-        const float sc = __ldg(s + i);
-        const float gx = 0.5f * (__ldg(s + i + (x < nx - 1 ? 1 : 0)) - __ldg(s + i - (x > 0 ? 1 : 0)));
-        const float gy = 0.5f * (__ldg(s + i + (y < ny - 1 ? (size_t)nx : 0)) - __ldg(s + i - (y > 0 ? (size_t)nx : 0)));
-        const float gz = 0.5f * (__ldg(s + i + (z < nz - 1 ? plane : 0)) - __ldg(s + i - (z > 0 ? plane : 0)));
-        const float d = sc - __ldg(m + i);
-        const float den = fmaf(gx, gx, fmaf(gy, gy, fmaf(gz, gz, fmaf(d, d, eps_den))));
-        const float q = __fdividef(d, den);
+    if (MODE != kForceNone) {
+        const size_t xp = i + (x < nx - 1 ? 1 : 0), xm = i - (x > 0 ? 1 : 0);
+        const size_t yp = i + (y < ny - 1 ? (size_t)nx : 0), ym = i - (y > 0 ? (size_t)nx : 0);
+        const size_t zp = i + (z < nz - 1 ? plane : 0), zm = i - (z > 0 ? plane : 0);
+        const float gx = 0.5f * (__ldg(s + xp) - __ldg(s + xm));
+        const float gy = 0.5f * (__ldg(s + yp) - __ldg(s + ym));
+        const float gz = 0.5f * (__ldg(s + zp) - __ldg(s + zm));
+        const float d = __ldg(s + i) - __ldg(m + i);
+        const float dd = fmaf(d, d, eps_den);
+        const float q = __fdividef(d, fmaf(gx, gx, fmaf(gy, gy, fmaf(gz, gz, dd))));
         out[0] = fmaf(q, gx, out[0]);
         out[1] = fmaf(q, gy, out[1]);
         out[2] = fmaf(q, gz, out[2]);
+        if (MODE == kForceDouble) {
+            const float hx = 0.5f * (__ldg(m + xp) - __ldg(m + xm));
+            const float hy = 0.5f * (__ldg(m + yp) - __ldg(m + ym));
+            const float hz = 0.5f * (__ldg(m + zp) - __ldg(m + zm));
+            const float p = __fdividef(d, fmaf(hx, hx, fmaf(hy, hy, fmaf(hz, hz, dd))));
+            out[0] = fmaf(p, hx, out[0]);
+            out[1] = fmaf(p, hy, out[1]);
+            out[2] = fmaf(p, hz, out[2]);
+        }
     }
 }
 
 // Step (c) alone, in place (disc_force_update).
-static __global__ void __launch_bounds__(256)
+template <int MODE>
+__global__ void __launch_bounds__(256)
 k_force_update(const float* __restrict__ m, const float* __restrict__ s, float* __restrict__ r, int nx, int ny,
                int nz, float eps_den) {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
@@ -50,13 +66,13 @@ k_force_update(const float* __restrict__ m, const float* __restrict__ s, float* 
     if (x >= nx) return;
     const size_t N = (size_t)nx * ny * nz;
     float u[3];
-    updated_field<true>(m, s, r, nx, ny, nz, N, x, y, z, eps_den, u);
+    updated_field<MODE>(m, s, r, nx, ny, nz, N, x, y, z, eps_den, u);
     const size_t i = ((size_t)z * ny + y) * nx + x;
     r[i] = u[0]; r[N + i] = u[1]; r[2 * N + i] = u[2];
 }
 
 // [force + update] + Gaussian x + Gaussian y.  Grid (x tiles, y segments, z); TXB threads <-> x.
-template <int K, bool FORCE, int TXB>
+template <int K, int FORCE, int TXB>
 __global__ void __launch_bounds__(TXB)
 k_force_gxy(const float* __restrict__ m, const float* __restrict__ s, const float* __restrict__ rin,
             float* __restrict__ rout, int nx, int ny, int nz, int yseg, float eps_den, GaussTaps gw) {

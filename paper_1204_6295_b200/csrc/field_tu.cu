@@ -13,7 +13,7 @@ namespace disc {
 
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-template <int K, bool FORCE>
+template <int K, int FORCE>
 static void launch_fg(int txb, const float* m, const float* s, const float* rin, float* rout, int nx, int ny, int nz,
                       int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
     const bool vec_ok = nx % 4 == 0 && aligned16(rin) && aligned16(rout) && (!FORCE || (aligned16(m) && aligned16(s)));
@@ -78,11 +78,12 @@ static void launch_gz(const float* rin, float* rout, const float* moving, float*
 
 // one Gaussian radius: launches if K lies in this unit's range (the discarded branch is never instantiated)
 template <int K>
-static bool case_fg(bool force, int txb, const float* m, const float* s, const float* rin, float* rout, int nx, int ny,
+static bool case_fg(int force, int txb, const float* m, const float* s, const float* rin, float* rout, int nx, int ny,
                     int nz, int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
     if constexpr (K >= DISC_K_LO && K <= DISC_K_HI) {
-        if (force) launch_fg<K, true>(txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
-        else launch_fg<K, false>(txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
+        if (force == kForceDouble) launch_fg<K, kForceDouble>(txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
+        else if (force == kForceSingle) launch_fg<K, kForceSingle>(txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
+        else launch_fg<K, kForceNone>(txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
         return true;
     } else {
         return false;
@@ -103,7 +104,7 @@ static bool case_gz(bool warp, const float* rin, float* rout, const float* movin
 
 #define DISC_FOR_K(X) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12)
 
-bool DISC_CAT(launch_force_gxy_tu, DISC_TU)(int K, bool force, int txb, const float* m, const float* s,
+bool DISC_CAT(launch_force_gxy_tu, DISC_TU)(int K, int force, int txb, const float* m, const float* s,
                                             const float* rin, float* rout, int nx, int ny, int nz, int yseg,
                                             float eps_den, const GaussTaps& taps, cudaStream_t st) {
     switch (K) {
@@ -128,10 +129,11 @@ bool DISC_CAT(launch_gz_warp_tu, DISC_TU)(int K, bool warp, const float* rin, fl
 }
 
 #if DISC_TU == 0
-void launch_force_update(const float* m, const float* s, float* r, int nx, int ny, int nz, float eps_den,
+void launch_force_update(int force, const float* m, const float* s, float* r, int nx, int ny, int nz, float eps_den,
                          cudaStream_t st) {
     dim3 grid((nx + 255) / 256, ny, nz);
-    k_force_update<<<grid, 256, 0, st>>>(m, s, r, nx, ny, nz, eps_den);
+    if (force == kForceDouble) k_force_update<kForceDouble><<<grid, 256, 0, st>>>(m, s, r, nx, ny, nz, eps_den);
+    else k_force_update<kForceSingle><<<grid, 256, 0, st>>>(m, s, r, nx, ny, nz, eps_den);
 }
 
 void launch_warp_kernel(const float* moving, const float* r, float* out, int nx, int ny, int nz, cudaStream_t st) {
@@ -147,7 +149,7 @@ bool launch_moments_any(int R, int mode, int ty, const float* vol, const float* 
            launch_moments_tu3(R, mode, ty, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st);
 }
 
-bool launch_force_gxy_any(int K, bool force, int txb, const float* m, const float* s, const float* rin, float* rout,
+bool launch_force_gxy_any(int K, int force, int txb, const float* m, const float* s, const float* rin, float* rout,
                           int nx, int ny, int nz, int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
     return launch_force_gxy_tu0(K, force, txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st) ||
            launch_force_gxy_tu1(K, force, txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st) ||

@@ -259,10 +259,12 @@ struct FgT4Cfg {
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 
 // updated field of one group of four x-adjacent points (gx % 4 == 0), loads first, arithmetic after
-template <bool FORCE>
+template <int FORCE>
 struct FgGroup {
     float4 u[3], sc, mm, syp, sym, szp, szm;
     float sl, sr;
+    float4 myp, mym, mzp, mzm;   // double force only: the moving image's neighbours
+    float ml, mr;
     __device__ __forceinline__ void load(const float* __restrict__ m, const float* __restrict__ s,
                                          const float* __restrict__ rin, int nx, int ny, int nz, size_t plane, size_t N,
                                          int gx, int gy, int z) {
@@ -274,6 +276,11 @@ struct FgGroup {
             sl = __ldg(s + i - (gx > 0 ? 1 : 0)); sr = __ldg(s + i + 3 + (gx + 4 < nx ? 1 : 0));
             syp = ldg4(s + i + (gy < ny - 1 ? (size_t)nx : 0)); sym = ldg4(s + i - (gy > 0 ? (size_t)nx : 0));
             szp = ldg4(s + i + (z < nz - 1 ? plane : 0)); szm = ldg4(s + i - (z > 0 ? plane : 0));
+            if (FORCE == kForceDouble) {
+                ml = __ldg(m + i - (gx > 0 ? 1 : 0)); mr = __ldg(m + i + 3 + (gx + 4 < nx ? 1 : 0));
+                myp = ldg4(m + i + (gy < ny - 1 ? (size_t)nx : 0)); mym = ldg4(m + i - (gy > 0 ? (size_t)nx : 0));
+                mzp = ldg4(m + i + (z < nz - 1 ? plane : 0)); mzm = ldg4(m + i - (z > 0 ? plane : 0));
+            }
         }
     }
     __device__ __forceinline__ void finish(float eps_den) {
@@ -284,17 +291,29 @@ struct FgGroup {
             const float zp[4] = {szp.x, szp.y, szp.z, szp.w}, zm[4] = {szm.x, szm.y, szm.z, szm.w};
             float ux[4] = {u[0].x, u[0].y, u[0].z, u[0].w}, uy[4] = {u[1].x, u[1].y, u[1].z, u[1].w};
             float uz[4] = {u[2].x, u[2].y, u[2].z, u[2].w};
+            const float he[6] = {ml, mm.x, mm.y, mm.z, mm.w, mr};
+            const float hyp[4] = {myp.x, myp.y, myp.z, myp.w}, hym[4] = {mym.x, mym.y, mym.z, mym.w};
+            const float hzp[4] = {mzp.x, mzp.y, mzp.z, mzp.w}, hzm[4] = {mzm.x, mzm.y, mzm.z, mzm.w};
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
                 const float gxv = 0.5f * (ce[e + 2] - ce[e]);
                 const float gyv = 0.5f * (yp[e] - ym[e]);
                 const float gzv = 0.5f * (zp[e] - zm[e]);
                 const float d = ce[e + 1] - me[e];
-                const float den = fmaf(gxv, gxv, fmaf(gyv, gyv, fmaf(gzv, gzv, fmaf(d, d, eps_den))));
-                const float q = __fdividef(d, den);
+                const float dd = fmaf(d, d, eps_den);
+                const float q = __fdividef(d, fmaf(gxv, gxv, fmaf(gyv, gyv, fmaf(gzv, gzv, dd))));
                 ux[e] = fmaf(q, gxv, ux[e]);
                 uy[e] = fmaf(q, gyv, uy[e]);
                 uz[e] = fmaf(q, gzv, uz[e]);
+                if (FORCE == kForceDouble) {
+                    const float hxv = 0.5f * (he[e + 2] - he[e]);
+                    const float hyv = 0.5f * (hyp[e] - hym[e]);
+                    const float hzv = 0.5f * (hzp[e] - hzm[e]);
+                    const float p = __fdividef(d, fmaf(hxv, hxv, fmaf(hyv, hyv, fmaf(hzv, hzv, dd))));
+                    ux[e] = fmaf(p, hxv, ux[e]);
+                    uy[e] = fmaf(p, hyv, uy[e]);
+                    uz[e] = fmaf(p, hzv, uz[e]);
+                }
             }
             u[0] = make_float4(ux[0], ux[1], ux[2], ux[3]);
             u[1] = make_float4(uy[0], uy[1], uy[2], uy[3]);
@@ -307,7 +326,7 @@ struct FgGroup {
 // running at the same time work on neighbouring tiles and share their halos in L2).  Phase 3 of tile t-1 and
 // phase 1 of tile t share one barrier interval -- the y pass (pure FMA work out of shared memory) runs on some
 // warps while others wait for phase 1's global loads.
-template <int K, bool FORCE>
+template <int K, int FORCE>
 __global__ void __launch_bounds__(FgT4Cfg<K>::NT, FgT4Cfg<K>::OCC)
 k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const float* __restrict__ rin,
                float* __restrict__ rout, int nx, int ny, int nz, float eps_den, GaussTaps gw) {

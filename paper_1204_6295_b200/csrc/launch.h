@@ -21,11 +21,12 @@ enum MomentsMode {
 
 bool launch_moments_any(int R, int mode, int ty, const float* vol, const float* aux, float* out0, float* out1, int nx,
                         int ny, int nz, int zchunk, float eps_var, cudaStream_t st);
-bool launch_force_gxy_any(int K, bool force, int txb, const float* m, const float* s, const float* rin, float* rout,
+// force = 0 none (plain smoothing), 1 Thirion / passive, 2 double (ForceMode in field.cuh)
+bool launch_force_gxy_any(int K, int force, int txb, const float* m, const float* s, const float* rin, float* rout,
                           int nx, int ny, int nz, int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st);
 bool launch_gz_warp_any(int K, bool warp, const float* rin, float* rout, const float* moving, float* mout, int nx,
                         int ny, int nz, int zchunk, const GaussTaps& taps, cudaStream_t st);
-void launch_force_update(const float* m, const float* s, float* r, int nx, int ny, int nz, float eps_den,
+void launch_force_update(int force, const float* m, const float* s, float* r, int nx, int ny, int nz, float eps_den,
                          cudaStream_t st);
 void launch_warp_kernel(const float* moving, const float* r, float* out, int nx, int ny, int nz, cudaStream_t st);
 
@@ -33,7 +34,7 @@ void launch_warp_kernel(const float* moving, const float* r, float* out, int nx,
 #define DISC_DECL_TU(n)                                                                                                  \
     bool launch_moments_tu##n(int R, int mode, int ty, const float* vol, const float* aux, float* out0, float* out1, int nx,     \
                               int ny, int nz, int zchunk, float eps_var, cudaStream_t st);                              \
-    bool launch_force_gxy_tu##n(int K, bool force, int txb, const float* m, const float* s, const float* rin,           \
+    bool launch_force_gxy_tu##n(int K, int force, int txb, const float* m, const float* s, const float* rin,           \
                                 float* rout, int nx, int ny, int nz, int yseg, float eps_den, const GaussTaps& taps,    \
                                 cudaStream_t st);                                                                        \
     bool launch_gz_warp_tu##n(int K, bool warp, const float* rin, float* rout, const float* moving, float* mout,        \

@@ -165,6 +165,34 @@ def test_demons_step(disc, oracle_mod, shape):
     assert np.abs(r.cpu().numpy() - ref).max() <= 1e-4
 
 
+# ------------------------------------------------------------------ double force (Eq. 1, both terms)
+@pytest.mark.parametrize("sigma", [1.5, 2.0, 3.0])
+@pytest.mark.parametrize("shape", SHAPES + [(40, 300, 152)])
+def test_double_force(disc, oracle_mod, shape, sigma):
+    m, s = rand_pair(shape, 70)
+    r0 = np.random.default_rng(71).normal(0, 1, size=(3,) + shape).astype(np.float32)
+    ctx = make_ctx(disc, shape, sigma=sigma)
+    disc.disc_set_force(ctx, disc.DISC_FORCE_DOUBLE)
+    r = dev(r0)
+    disc.disc_force_update(ctx, 0, dev(m), dev(s), r)
+    assert np.abs(r.cpu().numpy() - oracle_mod.force_update(m, s, r0, double_force=True)).max() <= 1e-4
+    r = dev(r0)
+    disc.disc_demons_step(ctx, 0, dev(m), dev(s), r)
+    assert np.abs(r.cpu().numpy() - oracle_mod.demons_step(m, s, r0, sigma, double_force=True)).max() <= 1e-4
+    # m = s: no force (bit exact); smoothing alone is unaffected by the mode
+    r = dev(r0)
+    disc.disc_force_update(ctx, 0, dev(s), dev(s), r)
+    assert np.array_equal(r.cpu().numpy(), r0)
+    # switching back restores the Thirion force
+    disc.disc_set_force(ctx, disc.DISC_FORCE_THIRION)
+    r = dev(r0)
+    disc.disc_demons_step(ctx, 0, dev(m), dev(s), r)
+    assert np.abs(r.cpu().numpy() - oracle_mod.demons_step(m, s, r0, sigma)).max() <= 1e-4
+    with pytest.raises(disc.DiscError):
+        disc.disc_set_force(ctx, 7)
+    disc.disc_destroy(ctx)
+
+
 # ------------------------------------------------------------------ pyramid
 @pytest.mark.parametrize("shape", [(4, 6, 8), (16, 34, 66), (2, 2, 2)])
 def test_pyramid(disc, oracle_mod, shape):

@@ -25,9 +25,11 @@ def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
 
 
-def gpu_register(disc, ct, cbct, R, sigma, levels, iters, host=False):
+def gpu_register(disc, ct, cbct, R, sigma, levels, iters, host=False, double_force=False):
     nz, ny, nx = ct.shape
     ctx = disc.disc_create((nx, ny, nz), (1.0, 1.0, 1.0), R, sigma, levels, iters)
+    if double_force:
+        disc.disc_set_force(ctx, disc.DISC_FORCE_DOUBLE)
     if host:
         r = np.empty((3,) + ct.shape, dtype=np.float32)
         corr = np.empty_like(ct)
@@ -102,3 +104,19 @@ def test_iterate_matches_stepwise_oracle(disc, oracle_mod):
         m = oracle_mod.warp(ct, rr)
         rr = oracle_mod.demons_step(m, oracle_mod.correct(cbct, m, R), rr, sigma)
     assert np.abs(d_r.cpu().numpy() - rr).max() <= 1e-3
+
+
+@pytest.mark.parametrize("dims,R,sigma,levels,iters", [
+    ((40, 36, 20), 2, 1.5, 2, 10),
+    ((64, 64, 32), 3, 1.5, 1, 50),       # config 1's schedule
+    ((70, 44, 24), 3, 2.0, 3, 8),
+])
+def test_register_double_force(disc, oracle_mod, dims, R, sigma, levels, iters):
+    """the whole schedule with both terms of Eq. (1)"""
+    dims = tuple(d - d % (1 << (levels - 1)) for d in dims)
+    ct, cbct, _, _ = phantoms.make_pair(1, dims=dims)
+    r, corr, _ = gpu_register(disc, ct, cbct, R, sigma, levels, iters, double_force=True)
+    r_ref, corr_ref = oracle_mod.register(ct, cbct, R, sigma, levels, iters, double_force=True)
+    check(ct, cbct, r, corr, r_ref, corr_ref)
+    r1, _ = oracle_mod.register(ct, cbct, R, sigma, levels, iters, want_corr=False)
+    assert np.abs(r_ref - r1).max() > 0.05      # and it is a different registration than the Thirion one
