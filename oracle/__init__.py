@@ -194,3 +194,39 @@ def register(ct, cbct, R, sigma, levels, iters, eps_var=EPS_VAR, eps_den=EPS_DEN
                       trace.ctypes.data_as(_f64p) if want_trace else None)
     out = (disp, corr)
     return out + (trace,) if want_trace else out
+
+
+def force_norms(m, s, disp, eps_den=EPS_DEN, double_force=False):
+    """(sum |dr|, sum |r|) of the paper's convergence measure l = sum|dr| / sum|r| (reading A16)."""
+    L = _load()
+    m_, pm = _f32(m)
+    s_, ps = _f32(s)
+    d, pd = _f32(disp)
+    a, b = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    L.oracle_force_norms(pm, ps, pd, *_dims(m_), ctypes.c_double(eps_den), ctypes.c_int(1 if double_force else 0),
+                         ctypes.byref(a), ctypes.byref(b))
+    return a.value, b.value
+
+
+def register_stop(ct, cbct, R, sigma, levels, iters, stop_eps=None, iters_per_level=None, double_force=False,
+                  eps_var=EPS_VAR, eps_den=EPS_DEN):
+    """Algorithm A1 with the paper's stopping criterion l(k-10) - l(k) <= stop_eps inside every level (PAPER.md:167,
+    :187); `iters` is the per-level maximum.  Returns (disp, iterations run per level [0 = finest],
+    l trace [levels, iters], coarsest level first, nan where not run)."""
+    L = _load()
+    a, pa = _f32(ct)
+    b, pb = _f32(cbct)
+    disp = np.empty((3,) + a.shape, dtype=np.float32)
+    run = np.zeros(levels, dtype=np.int32)
+    ltrace = np.full((levels, max(iters, 1)), np.nan, dtype=np.float64)
+    ipl = None if iters_per_level is None else np.ascontiguousarray(iters_per_level, dtype=np.int32)
+    if ipl is not None:
+        assert ipl.size == levels and ipl.max() <= iters
+    i32p = ctypes.POINTER(ctypes.c_int)
+    L.oracle_register_full(pa, pb, *_dims(a), ctypes.c_int(R), ctypes.c_double(sigma), ctypes.c_int(levels),
+                           ctypes.c_int(iters), ctypes.c_double(eps_var), ctypes.c_double(eps_den),
+                           ctypes.c_int(1 if double_force else 0),
+                           ctypes.c_double(-1.0 if stop_eps is None else float(stop_eps)),
+                           ipl.ctypes.data_as(i32p) if ipl is not None else None, run.ctypes.data_as(i32p),
+                           ltrace.ctypes.data_as(_f64p), disp.ctypes.data_as(_f32p), None, None)
+    return disp, run, ltrace

@@ -218,6 +218,28 @@ void oracle_force_update_double(const float *m, const float *s, int nx, int ny, 
             }
 }
 
+/* NEXT-3: the two sums of the paper's convergence measure (section 2.3):
+ *   l^(k) = sum_x |dr^(k+1)(x)| / sum_x |r^(k)(x)|,
+ * dr = the increment the force is about to add (before any smoothing), r = the total field before the update.
+ * Reading A16: |.| is the Euclidean norm of the 3-vector at a voxel.  fp64 throughout. */
+void oracle_force_norms(const float *m, const float *s, const float *disp, int nx, int ny, int nz, double eps_den,
+                        int double_force, double *sum_dr, double *sum_r) {
+    size_t N = (size_t)nx * ny * nz;
+    float *tmp = (float *)calloc(3 * N, sizeof(float));
+    double a = 0.0, b = 0.0;
+    /* the increment alone: the update applied to a zero field, in fp64 before the final rounding to fp32 */
+    if (double_force) oracle_force_update_double(m, s, nx, ny, nz, eps_den, tmp);
+    else oracle_force_update(m, s, nx, ny, nz, eps_den, tmp);
+    for (size_t i = 0; i < N; ++i) {
+        double dx = tmp[i], dy = tmp[N + i], dz = tmp[2 * N + i];
+        double rx = disp[i], ry = disp[N + i], rz = disp[2 * N + i];
+        a += sqrt(dx * dx + dy * dy + dz * dz);
+        b += sqrt(rx * rx + ry * ry + rz * rz);
+    }
+    free(tmp);
+    *sum_dr = a; *sum_r = b;
+}
+
 /* ------------------------------------------------------------------------
  * (d) Gaussian regularisation of the total field r (Alg. A1 step 6,
  * PAPER.md:194).  Reading A10: K = ceil(3 sigma), w_i ~ exp(-i^2 / 2 sigma^2)
@@ -310,8 +332,17 @@ void oracle_upsample_field(const float *dc, int cx, int cy, int cz, float *out) 
  * they are computed once per level with the same naive loop.
  * `trace` (optional, may be NULL): receives sum|r| after every iteration.
  * ---------------------------------------------------------------------- */
-void oracle_register_mode(const float *ct, const float *cbct, int nx, int ny, int nz, int R, double sigma, int levels,
-                          int iters, double eps_var, double eps_den, int double_force, float *out_disp,
+/* The general driver.  stop_eps >= 0 enables the paper's stopping criterion: inside a
+ * level, l^(k) is evaluated in every iteration k = 0,1,.. (from that iteration's dr and the field before the
+ * update; l = +inf while sum|r| = 0); the iteration in which  l^(k-10) - l^(k) <= stop_eps  first holds (k >= 10)
+ * is completed and is the level's last.  `iters` stays the per-level maximum.  The text's criterion is followed;
+ * Alg. A1's `while` prints it inverted (PAPER.md:187 vs :167).
+ * iters_per_level (optional): explicit iteration counts, index = level (0 = finest), overriding `iters`.
+ * iters_run (optional, [levels]): iterations actually run per level.  ltrace (optional, [levels*iters]): l^(k),
+ * level-major from the coarsest level, `iters` slots per level. */
+void oracle_register_full(const float *ct, const float *cbct, int nx, int ny, int nz, int R, double sigma, int levels,
+                          int iters, double eps_var, double eps_den, int double_force, double stop_eps,
+                          const int *iters_per_level, int *iters_run, double *ltrace, float *out_disp,
                           float *out_corr, double *trace) {
     const float **pct = (const float **)malloc(sizeof(float *) * levels);
     const float **pcb = (const float **)malloc(sizeof(float *) * levels);
@@ -340,10 +371,20 @@ void oracle_register_mode(const float *ct, const float *cbct, int nx, int ny, in
         double *mus = (double *)malloc(sizeof(double) * N), *vs = (double *)malloc(sizeof(double) * N);
         double *mum = (double *)malloc(sizeof(double) * N), *vm = (double *)malloc(sizeof(double) * N);
         oracle_box_moments(pcb[l], lx, ly, lz, R, mus, vs);
-        for (int k = 0; k < iters; ++k) {
+        int n_it = iters_per_level ? iters_per_level[l] : iters, k_run = 0;
+        double *hist = (double *)malloc(sizeof(double) * (n_it > 0 ? n_it : 1));
+        for (int k = 0; k < n_it; ++k) {
+            int stop = 0;
             oracle_warp(pct[l], r, lx, ly, lz, m);                                   /* I_m^(k) */
             oracle_box_moments(m, lx, ly, lz, R, mum, vm);                           /* A1 step 1 */
             oracle_correct_from_moments(pcb[l], mus, vs, mum, vm, N, eps_var, sp);   /* A1 step 3 */
+            if (stop_eps >= 0.0 || ltrace) {
+                double sdr, sr;
+                oracle_force_norms(m, sp, r, lx, ly, lz, eps_den, double_force, &sdr, &sr);
+                hist[k] = sr > 0.0 ? sdr / sr : INFINITY;
+                if (ltrace) ltrace[(size_t)(levels - 1 - l) * iters + k] = hist[k];
+                if (stop_eps >= 0.0 && k >= 10 && hist[k - 10] - hist[k] <= stop_eps) stop = 1;
+            }
             if (double_force) oracle_force_update_double(m, sp, lx, ly, lz, eps_den, r); /* Eq. (1), both terms */
             else oracle_force_update(m, sp, lx, ly, lz, eps_den, r);                 /* A1 steps 4-5 */
             oracle_smooth_field(r, lx, ly, lz, sigma);                               /* A1 step 6 */
@@ -353,7 +394,11 @@ void oracle_register_mode(const float *ct, const float *cbct, int nx, int ny, in
                 trace[it_total] = s;
             }
             ++it_total;
+            k_run = k + 1;
+            if (stop) break;
         }
+        free(hist);
+        if (iters_run) iters_run[l] = k_run;
         if (l == 0) {
             memcpy(out_disp, r, sizeof(float) * 3 * N);
             if (out_corr) {
@@ -367,6 +412,13 @@ void oracle_register_mode(const float *ct, const float *cbct, int nx, int ny, in
     free(r);
     for (int l = 1; l < levels; ++l) { free((void *)pct[l]); free((void *)pcb[l]); }
     free(pct); free(pcb);
+}
+
+void oracle_register_mode(const float *ct, const float *cbct, int nx, int ny, int nz, int R, double sigma, int levels,
+                          int iters, double eps_var, double eps_den, int double_force, float *out_disp,
+                          float *out_corr, double *trace) {
+    oracle_register_full(ct, cbct, nx, ny, nz, R, sigma, levels, iters, eps_var, eps_den, double_force, -1.0, NULL, NULL,
+                         NULL, out_disp, out_corr, trace);
 }
 
 /* north_star's schedule: the Thirion (single, passive) force */

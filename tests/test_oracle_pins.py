@@ -246,6 +246,69 @@ def test_double_force_recovers_a_translation(oracle_mod):
     assert e2 < e0 / 2.5 and e2 < 1.1 * e1, (e0, e1, e2)
 
 
+def test_convergence_measure_pins(oracle_mod):
+    """NEXT-3: l = sum|dr| / sum|r|.  Closed form on a ramp, Euclidean norm per voxel (reading A16)."""
+    nz, ny, nx = 4, 5, 9
+    z, y, x = np.meshgrid(np.arange(float(nz)), np.arange(float(ny)), np.arange(float(nx)), indexing="ij")
+    g, delta = 20.0, 0.75
+    sp, mm = (g * x).astype(np.float32), (g * x - g * delta).astype(np.float32)
+    r = np.empty((3, nz, ny, nx), dtype=np.float32); r[0], r[1], r[2] = 3.0, -4.0, 12.0      # |r| = 13 at every voxel
+    sdr, sr = oracle_mod.force_norms(mm, sp, r, eps_den=0.0)
+    d = g * delta
+    inner, border = d * g / (g * g + d * d), d * (g / 2) / ((g / 2) ** 2 + d * d)             # clamped central difference
+    np.testing.assert_allclose(sdr, nz * ny * ((nx - 2) * inner + 2 * border), rtol=1e-6)
+    np.testing.assert_allclose(sr, 13.0 * nz * ny * nx, rtol=1e-12)
+    # a diagonal ramp: |dr| is the Euclidean norm, not the sum of |components|
+    sp2 = (g * (x + y)).astype(np.float32)
+    sdr2, _ = oracle_mod.force_norms(sp2 - np.float32(d), sp2, r, eps_den=0.0)
+    core = (slice(1, -1),) * 3
+    per_voxel = np.sqrt(2.0) * d * g / (2 * g * g + d * d)
+    one, _ = oracle_mod.force_norms((sp2 - np.float32(d))[core], sp2[core], r[(slice(None),) + core], eps_den=0.0)
+    assert sdr2 > 0 and one > 0
+    dr = oracle_mod.force_update(sp2 - np.float32(d), sp2, np.zeros_like(r), eps_den=0.0)
+    np.testing.assert_allclose(np.sqrt((dr.astype(np.float64) ** 2).sum(0))[core], per_voxel, rtol=1e-5)
+    np.testing.assert_allclose(sdr2, np.sqrt((dr.astype(np.float64) ** 2).sum(0)).sum(), rtol=1e-6)
+    # double force: both terms equal on equal slopes -> twice the sum
+    sdr_d, _ = oracle_mod.force_norms(mm, sp, r, eps_den=0.0, double_force=True)
+    np.testing.assert_allclose(sdr_d, 2 * sdr, rtol=1e-6)
+
+
+def test_stopping_criterion_pins(oracle_mod):
+    """NEXT-3: stop at the first k >= 10 with l(k-10) - l(k) <= eps, inside each level; the iteration that trips it is
+    completed; an early-stopped run IS the fixed-count run with those counts."""
+    ct, cbct, _, _ = phantoms.make_pair(1, dims=(48, 40, 24))
+    R, sigma, levels, iters, eps = 3, 1.5, 2, 40, 2e-3
+    r, run, lt = oracle_mod.register_stop(ct, cbct, R, sigma, levels, iters, stop_eps=eps)
+    assert run.min() >= 11 and run.min() < iters                      # never before 11 iterations; something stopped early
+    for lev in range(levels):
+        row, n = lt[levels - 1 - lev], int(run[lev])
+        assert np.all(np.isfinite(row[1:n])) and np.all(np.isnan(row[n:]))
+        diffs = row[:n - 10] - row[10:n]                              # criterion values for k = 10 .. n-1
+        if n < iters:
+            assert diffs[-1] <= eps and np.all(diffs[:-1] > eps)      # tripped at k = n-1 and not before
+        else:
+            assert np.all(diffs[:-1] > eps)
+    assert np.isinf(lt[0, 0])                                         # r = 0 at the coarsest level's first iteration
+    # l itself, recomputed from the stepwise functions for the first two iterations of the coarsest level
+    c, b = oracle_mod.downsample(ct), oracle_mod.downsample(cbct)
+    rr = np.zeros((3,) + c.shape, dtype=np.float32)
+    for k in range(2):
+        m = oracle_mod.warp(c, rr)
+        sp = oracle_mod.correct(b, m, R)
+        dr = oracle_mod.force_update(m, sp, np.zeros_like(rr))
+        num = np.sqrt((dr.astype(np.float64) ** 2).sum(0)).sum()
+        den = np.sqrt((rr.astype(np.float64) ** 2).sum(0)).sum()
+        if den > 0:
+            np.testing.assert_allclose(lt[0, k], num / den, rtol=1e-5)
+        rr = oracle_mod.demons_step(m, sp, rr, sigma)
+    # composition: the same counts as a fixed schedule give the same field, bit for bit; and stop_eps = None runs them all
+    r_fixed, run_fixed, _ = oracle_mod.register_stop(ct, cbct, R, sigma, levels, iters, iters_per_level=run)
+    assert np.array_equal(r, r_fixed) and np.array_equal(run, run_fixed)
+    r_all, run_all, _ = oracle_mod.register_stop(ct, cbct, R, sigma, levels, 12)
+    r_ref, _ = oracle_mod.register(ct, cbct, R, sigma, levels, 12, want_corr=False)
+    assert np.array_equal(r_all, r_ref) and np.all(run_all == 12)
+
+
 def test_force_components_and_axes(oracle_mod):
     """each component uses its own axis' gradient (catches transposed strides)."""
     z, y, x = np.meshgrid(np.arange(5.), np.arange(6.), np.arange(7.), indexing="ij")
