@@ -90,6 +90,23 @@ unsigned long long disc_launch_count(const disc_ctx* ctx);
 #define DISC_FORCE_DOUBLE 2
 disc_status disc_set_force(disc_ctx* ctx, int mode);
 
+/* Stopping criterion of the paper (Alg. A1 :187), used by disc_iterate and disc_register
+ * from now on.  eps >= 0 enables it, eps < 0 disables it (default: fixed iteration counts, north_star).
+ * Inside a level, every iteration k = 0,1,.. evaluates  l(k) = sum_x |dr(x)| / sum_x |r(x)|  from the increment that
+ * iteration's force is about to add and the field before the update (Euclidean norm per voxel, reading A16;
+ * l = +inf while the field is zero).  The first iteration k >= 10 with  l(k-10) - l(k) <= eps  is completed and is the
+ * level's last; `iters` of disc_create stays the per-level maximum.  (The text's condition is followed; Alg. A1's
+ * `while` prints it inverted.)  The paper's value is eps = 1e-4.
+ * The test runs on the device: one extra launch per iteration (the paper's "comparison kernel", reading m, s', r once
+ * more: +20 B/voxel) whose last block sets a flag; the kernels of the remaining iterations are still enqueued but
+ * return at once, so there is no host synchronisation.  Host-side state only, no launch. */
+disc_status disc_set_stop(disc_ctx* ctx, float eps);
+
+/* Iterations actually run per level by the last disc_register / disc_iterate on this context:
+ * out_host[level], level = 0 .. levels-1 (HOST array of `levels` ints).  SYNCHRONISES the device when the
+ * stopping criterion is enabled; without it the counts are the requested ones. */
+disc_status disc_iterations_run(disc_ctx* ctx, int* out_host);
+
 /* ---- the steps of one iteration, in execution order b -> a -> c+d (Alg. A1) ---- */
 
 /* (b) out(x) = moving(x + disp(x)), trilinear, sample position clamped to the volume

@@ -23,7 +23,7 @@ DISC_EPS_DEN = 1e-3
 DISC_FORCE_THIRION, DISC_FORCE_DOUBLE = 1, 2
 
 EXPORTS = (
-    "disc_create", "disc_destroy", "disc_last_error", "disc_launch_count", "disc_set_force", "disc_warp", "disc_correct_intensity",
+    "disc_create", "disc_destroy", "disc_last_error", "disc_launch_count", "disc_set_force", "disc_set_stop", "disc_iterations_run", "disc_warp", "disc_correct_intensity",
     "disc_demons_step", "disc_register", "disc_register_host", "disc_iterate", "disc_box_moments",
     "disc_force_update", "disc_smooth_field", "disc_downsample", "disc_upsample_field", "disc_profile_iteration",
 )
@@ -46,6 +46,10 @@ _lib.disc_launch_count.restype = ctypes.c_ulonglong
 _lib.disc_launch_count.argtypes = [_vp]
 _lib.disc_set_force.restype = _i
 _lib.disc_set_force.argtypes = [_vp, _i]
+_lib.disc_set_stop.restype = _i
+_lib.disc_set_stop.argtypes = [_vp, ctypes.c_float]
+_lib.disc_iterations_run.restype = _i
+_lib.disc_iterations_run.argtypes = [_vp, ctypes.POINTER(_i)]
 for _name, _nptr in (("disc_warp", 3), ("disc_correct_intensity", 3), ("disc_demons_step", 3),
                      ("disc_box_moments", 3), ("disc_force_update", 3), ("disc_smooth_field", 1),
                      ("disc_downsample", 2), ("disc_upsample_field", 2)):
@@ -157,6 +161,17 @@ def disc_launch_count(ctx: Ctx) -> int:
 
 def disc_set_force(ctx, mode):
     _check(ctx.handle, _lib.disc_set_force(ctx.handle, int(mode)))
+
+
+def disc_set_stop(ctx, eps):
+    _check(ctx.handle, _lib.disc_set_stop(ctx.handle, float(eps)))
+
+
+def disc_iterations_run(ctx):
+    """iterations run per level (index = level) by the last disc_register / disc_iterate; synchronises"""
+    out = (_i * ctx.levels)()
+    _check(ctx.handle, _lib.disc_iterations_run(ctx.handle, out))
+    return [int(v) for v in out]
 
 
 def disc_warp(ctx, level, moving, disp, out, stream=None):

@@ -16,6 +16,24 @@ struct Dims {
     int nx, ny, nz;
 };
 
+// Stopping criterion: device-side state of one context.  Every kernel of iteration
+// `iter` gets an IterCtl by value and returns at once when iter > *stop_iter, so an early stop needs no host
+// synchronisation: the remaining launches of the level fall through.  stop_iter == nullptr: criterion off.
+struct StopCtl {
+    double sum_dr, sum_r;      // accumulators of the running iteration
+    double hist[16];           // l^(k) of the last 16 iterations, slot k & 15
+    unsigned ticket;           // blocks of k_force_norms finished
+    int stop_iter;             // last iteration of the level (INT_MAX while running)
+    int runs[8];               // iterations run per level (DISC_MAX_LEVELS)
+};
+struct IterCtl {
+    const int* stop_iter;
+    int iter;
+};
+__device__ __forceinline__ bool iter_skipped(const IterCtl& c) {
+    return c.stop_iter != nullptr && c.iter > *reinterpret_cast<const volatile int*>(c.stop_iter);
+}
+
 __device__ __forceinline__ int clampi(int v, int lo, int hi) { return min(max(v, lo), hi); }
 
 // Trilinear sample of I at (px,py,pz), position clamped to the volume (reading A11):

@@ -32,6 +32,10 @@ thread_local char g_create_error[256] = "";
 
 }  // namespace
 
+namespace disc {
+thread_local IterCtl g_iter_ctl = {nullptr, 0};
+}
+
 struct disc_ctx {
     int dims[3];
     float spacing[3];
@@ -40,6 +44,9 @@ struct disc_ctx {
     int levels, iters;
     int K;
     int force_mode;   // 1 Thirion (default), 2 double force
+    float stop_eps;   // < 0: stopping criterion off (default)
+    StopCtl* d_stop;  // device-side state of the criterion
+    int runs_host[DISC_MAX_LEVELS];   // iterations per level when the criterion is off
     int n_sm;
     GaussTaps taps;
     Level lv[DISC_MAX_LEVELS];
@@ -182,15 +189,32 @@ disc_status launch_upsample(disc_ctx* c, const Level& coarse, const float* in, f
 // With final_warp the last iteration also refreshes L.m (needed when the caller goes on using it).
 disc_status iterate_level(disc_ctx* c, Level& L, const float* ct, float* disp, int n_iters, bool final_warp,
                           cudaStream_t st) {
-    for (int k = 0; k < n_iters; ++k) {
-        DISC_TRY(launch_moments<kModeCorrect>(c, L, L.m, L.zhat, L.sp, nullptr, st));       // A1 steps 1,3
-        DISC_TRY(launch_force_gxy(c, true, L, L.m, L.sp, disp, L.scratch, st));              // A1 steps 4,5,6(x,y)
-        if (k + 1 < n_iters || final_warp)
-            DISC_TRY(launch_gz_warp<true>(c, L, L.scratch, disp, ct, L.m, st));              // A1 step 6(z) + next I_m^(k)
-        else
-            DISC_TRY(launch_gz_warp<false>(c, L, L.scratch, disp, nullptr, nullptr, st));
+    const int level = (int)(&L - c->lv);
+    const bool stop = c->stop_eps >= 0.f;
+    c->runs_host[level] = n_iters;
+    if (stop) { launch_stop_reset(c->d_stop, st); DISC_TRY(check_launch(c, "k_stop_reset")); }
+    disc_status rc = DISC_OK;
+    for (int k = 0; k < n_iters && rc == DISC_OK; ++k) {
+        // with the criterion on, every kernel of iteration k falls through once an earlier iteration has tripped it;
+        // the field and L.m then stay those of the last iteration run (its z pass always refreshes L.m: k + 1 < n_iters)
+        g_iter_ctl = stop ? IterCtl{&c->d_stop->stop_iter, k} : IterCtl{nullptr, 0};
+        rc = launch_moments<kModeCorrect>(c, L, L.m, L.zhat, L.sp, nullptr, st);              // A1 steps 1,3
+        if (rc == DISC_OK && stop) {                                                           // PAPER.md:167, l^(k)
+            launch_force_norms(c->force_mode, L.m, L.sp, disp, L.nx, L.ny, L.nz, DISC_EPS_DEN, c->d_stop, k, c->stop_eps,
+                               c->n_sm, st);
+            rc = check_launch(c, "k_force_norms");
+        }
+        if (rc == DISC_OK) rc = launch_force_gxy(c, true, L, L.m, L.sp, disp, L.scratch, st);  // A1 steps 4,5,6(x,y)
+        if (rc == DISC_OK) {
+            if (k + 1 < n_iters || final_warp)
+                rc = launch_gz_warp<true>(c, L, L.scratch, disp, ct, L.m, st);                 // A1 step 6(z) + next I_m^(k)
+            else
+                rc = launch_gz_warp<false>(c, L, L.scratch, disp, nullptr, nullptr, st);
+        }
     }
-    return DISC_OK;
+    g_iter_ctl = IterCtl{nullptr, 0};
+    if (rc == DISC_OK && stop) { launch_stop_record(c->d_stop, level, n_iters, st); rc = check_launch(c, "k_stop_record"); }
+    return rc;
 }
 
 void free_ctx(disc_ctx* c) {
@@ -199,6 +223,7 @@ void free_ctx(disc_ctx* c) {
         cudaFree(L.ct); cudaFree(L.cbct); cudaFree(L.zhat); cudaFree(L.m); cudaFree(L.sp);
         cudaFree(L.disp); cudaFree(L.scratch);
     }
+    cudaFree(c->d_stop);
     cudaFree(c->h2d_ct); cudaFree(c->h2d_cbct); cudaFree(c->d_out_disp); cudaFree(c->d_out_corr);
     delete c;
 }
@@ -245,6 +270,12 @@ disc_status disc_create(disc_ctx** out, const int dims[3], const float spacing[3
     cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
     c->R = patch_radius; c->sigma = sigma_smooth; c->levels = levels; c->iters = iters; c->K = K;
     c->force_mode = DISC_FORCE_THIRION;
+    c->stop_eps = -1.f;
+    if (cudaMalloc(&c->d_stop, sizeof(StopCtl)) != cudaSuccess || cudaMemset(c->d_stop, 0, sizeof(StopCtl)) != cudaSuccess) {
+        cudaGetLastError();
+        free_ctx(c);
+        return fail(nullptr, DISC_ERR_ALLOC, "cudaMalloc failed (stop control)");
+    }
     // Gaussian taps: fp64, normalised to sum 1, then rounded to fp32 (reading A10)
     {
         double w[kMaxGaussTaps], sum = 0.0;
@@ -285,6 +316,28 @@ disc_status disc_set_force(disc_ctx* c, int mode) {
     if (!c) return DISC_ERR_INVALID_ARG;
     DISC_NEED(c, mode == DISC_FORCE_THIRION || mode == DISC_FORCE_DOUBLE, "force mode must be DISC_FORCE_THIRION or DISC_FORCE_DOUBLE");
     c->force_mode = mode;
+    return DISC_OK;
+}
+
+disc_status disc_set_stop(disc_ctx* c, float eps) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_NEED(c, eps == eps, "eps is NaN");
+    c->stop_eps = eps >= 0.f ? eps : -1.f;
+    return DISC_OK;
+}
+
+disc_status disc_iterations_run(disc_ctx* c, int* out_host) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_NEED(c, out_host, "NULL pointer");
+    if (c->stop_eps >= 0.f) {
+        StopCtl h;
+        cudaError_t e = cudaDeviceSynchronize();
+        if (e == cudaSuccess) e = cudaMemcpy(&h, c->d_stop, sizeof(h), cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return fail(c, DISC_ERR_CUDA, "reading the stop control: %s", cudaGetErrorString(e));
+        for (int l = 0; l < c->levels; ++l) out_host[l] = h.runs[l];
+    } else {
+        for (int l = 0; l < c->levels; ++l) out_host[l] = c->runs_host[l];
+    }
     return DISC_OK;
 }
 

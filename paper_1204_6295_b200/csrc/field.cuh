@@ -56,6 +56,83 @@ __device__ __forceinline__ void updated_field(const float* __restrict__ m, const
     }
 }
 
+// The increment alone (no field): dr_c = d g_c / (|g|^2 + d^2 + eps) [+ d h_c / (|h|^2 + d^2 + eps)].
+template <int MODE>
+__device__ __forceinline__ void force_increment(const float* __restrict__ m, const float* __restrict__ s, int nx, int ny,
+                                                int nz, int x, int y, int z, float eps_den, float dr[3]) {
+    const size_t plane = (size_t)nx * ny;
+    const size_t i = (size_t)z * plane + (size_t)y * nx + x;
+    const size_t xp = i + (x < nx - 1 ? 1 : 0), xm = i - (x > 0 ? 1 : 0);
+    const size_t yp = i + (y < ny - 1 ? (size_t)nx : 0), ym = i - (y > 0 ? (size_t)nx : 0);
+    const size_t zp = i + (z < nz - 1 ? plane : 0), zm = i - (z > 0 ? plane : 0);
+    const float gx = 0.5f * (__ldg(s + xp) - __ldg(s + xm));
+    const float gy = 0.5f * (__ldg(s + yp) - __ldg(s + ym));
+    const float gz = 0.5f * (__ldg(s + zp) - __ldg(s + zm));
+    const float d = __ldg(s + i) - __ldg(m + i);
+    const float dd = fmaf(d, d, eps_den);
+    const float q = __fdividef(d, fmaf(gx, gx, fmaf(gy, gy, fmaf(gz, gz, dd))));
+    dr[0] = q * gx; dr[1] = q * gy; dr[2] = q * gz;
+    if (MODE == kForceDouble) {
+        const float hx = 0.5f * (__ldg(m + xp) - __ldg(m + xm));
+        const float hy = 0.5f * (__ldg(m + yp) - __ldg(m + ym));
+        const float hz = 0.5f * (__ldg(m + zp) - __ldg(m + zm));
+        const float p = __fdividef(d, fmaf(hx, hx, fmaf(hy, hy, fmaf(hz, hz, dd))));
+        dr[0] = fmaf(p, hx, dr[0]); dr[1] = fmaf(p, hy, dr[1]); dr[2] = fmaf(p, hz, dr[2]);
+    }
+}
+
+// NEXT-3, the paper's "comparison kernel": sum_x |dr(x)| and sum_x |r(x)| (Euclidean norm per
+// voxel, reading A16) of iteration `iter`, per-thread fp32 norms accumulated in fp64; the last block to finish forms
+// l = sum|dr| / sum|r| (+inf while the field is zero), files it in the 16-slot history and, from iteration 10 on,
+// sets stop_iter = iter when l(iter-10) - l(iter) <= stop_eps.  Kernels of later iterations then fall through.
+template <int MODE>
+__global__ void __launch_bounds__(256)
+k_force_norms(const float* __restrict__ m, const float* __restrict__ s, const float* __restrict__ r, int nx, int ny,
+              int nz, float eps_den, StopCtl* ctl, int iter, float stop_eps) {
+    if (iter > *reinterpret_cast<volatile int*>(&ctl->stop_iter)) return;
+    const size_t N = (size_t)nx * ny * nz;
+    double a = 0.0, b = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
+        const int x = (int)(i % nx), y = (int)((i / nx) % ny), z = (int)(i / ((size_t)nx * ny));
+        float dr[3];
+        force_increment<MODE>(m, s, nx, ny, nz, x, y, z, eps_den, dr);
+        const float rx = __ldg(r + i), ry = __ldg(r + N + i), rz = __ldg(r + 2 * N + i);
+        a += (double)sqrtf(fmaf(dr[0], dr[0], fmaf(dr[1], dr[1], dr[2] * dr[2])));
+        b += (double)sqrtf(fmaf(rx, rx, fmaf(ry, ry, rz * rz)));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_xor_sync(0xffffffffu, a, o);
+        b += __shfl_xor_sync(0xffffffffu, b, o);
+    }
+    __shared__ double sh[2][8];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) { sh[0][warp] = a; sh[1][warp] = b; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double ta = 0.0, tb = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { ta += sh[0][w]; tb += sh[1][w]; }
+        atomicAdd(&ctl->sum_dr, ta);
+        atomicAdd(&ctl->sum_r, tb);
+        __threadfence();
+        if (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1) {
+            const double sdr = atomicAdd(&ctl->sum_dr, 0.0), sr = atomicAdd(&ctl->sum_r, 0.0);
+            const double l = sr > 0.0 ? sdr / sr : (double)INFINITY;
+            ctl->hist[iter & 15] = l;
+            if (iter >= 10 && ctl->hist[(iter - 10) & 15] - l <= (double)stop_eps) ctl->stop_iter = iter;
+            ctl->sum_dr = 0.0; ctl->sum_r = 0.0; ctl->ticket = 0u;
+            __threadfence();
+        }
+    }
+}
+
+static __global__ void k_stop_reset(StopCtl* ctl) {
+    ctl->sum_dr = 0.0; ctl->sum_r = 0.0; ctl->ticket = 0u; ctl->stop_iter = 0x7fffffff;
+}
+static __global__ void k_stop_record(StopCtl* ctl, int level, int n_iters) {
+    ctl->runs[level] = ctl->stop_iter == 0x7fffffff ? n_iters : ctl->stop_iter + 1;
+}
+
 // Step (c) alone, in place (disc_force_update).
 template <int MODE>
 __global__ void __launch_bounds__(256)
@@ -75,7 +152,8 @@ k_force_update(const float* __restrict__ m, const float* __restrict__ s, float* 
 template <int K, int FORCE, int TXB>
 __global__ void __launch_bounds__(TXB)
 k_force_gxy(const float* __restrict__ m, const float* __restrict__ s, const float* __restrict__ rin,
-            float* __restrict__ rout, int nx, int ny, int nz, int yseg, float eps_den, GaussTaps gw) {
+            float* __restrict__ rout, int nx, int ny, int nz, int yseg, float eps_den, GaussTaps gw, IterCtl ctl) {
+    if (iter_skipped(ctl)) return;
     constexpr int W = 2 * K + 1;
     __shared__ float row[2][3][TXB + 2 * K];
     const int tid = threadIdx.x;

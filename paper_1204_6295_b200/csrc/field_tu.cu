@@ -32,16 +32,16 @@ static void launch_fg(int txb, const float* m, const float* s, const float* rin,
         }
         const long long n_tiles = (long long)((nx + C::TX - 1) / C::TX) * ((ny + C::TY - 1) / C::TY) * nz;
         const int grid = (int)(n_tiles < (long long)C::OCC * n_sm ? n_tiles : (long long)C::OCC * n_sm);   // persistent: OCC CTAs per SM
-        k_force_gxy_t4<K, FORCE><<<grid, C::NT, C::smem_bytes, st>>>(m, s, rin, rout, nx, ny, nz, eps_den, taps);
+        k_force_gxy_t4<K, FORCE><<<grid, C::NT, C::smem_bytes, st>>>(m, s, rin, rout, nx, ny, nz, eps_den, taps, g_iter_ctl);
         return;
     }
     dim3 grid((nx + txb - 1) / txb, (ny + yseg - 1) / yseg, nz);
     if (txb == 128)
-        k_force_gxy<K, FORCE, 128><<<grid, 128, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps);
+        k_force_gxy<K, FORCE, 128><<<grid, 128, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, g_iter_ctl);
     else if (txb == 64)
-        k_force_gxy<K, FORCE, 64><<<grid, 64, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps);
+        k_force_gxy<K, FORCE, 64><<<grid, 64, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, g_iter_ctl);
     else
-        k_force_gxy<K, FORCE, 32><<<grid, 32, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps);
+        k_force_gxy<K, FORCE, 32><<<grid, 32, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, g_iter_ctl);
 }
 
 template <int K, bool WARP, int LZ>
@@ -49,7 +49,7 @@ static void launch_gzd(const float* rin, float* rout, const float* moving, float
                        const GaussTaps& taps, cudaStream_t st) {
     const size_t plane = (size_t)nx * ny;
     dim3 grid((unsigned)((plane + kGzdThreads - 1) / kGzdThreads), (nz + LZ - 1) / LZ, 1);
-    k_gz_warp_d<K, WARP, LZ><<<grid, kGzdThreads, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, taps);
+    k_gz_warp_d<K, WARP, LZ><<<grid, kGzdThreads, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, taps, g_iter_ctl);
 }
 
 template <int K, bool WARP, int LZ>
@@ -57,7 +57,7 @@ static void launch_gzd2(const float* rin, float* rout, const float* moving, floa
                         const GaussTaps& taps, cudaStream_t st) {
     const size_t pairs = (size_t)nx * ny / 2;
     dim3 grid((unsigned)((pairs + kGzdThreads - 1) / kGzdThreads), (nz + LZ - 1) / LZ, 1);
-    k_gz_warp_d2<K, WARP, LZ><<<grid, kGzdThreads, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, taps);
+    k_gz_warp_d2<K, WARP, LZ><<<grid, kGzdThreads, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, taps, g_iter_ctl);
 }
 
 static inline bool aligned8(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 7u) == 0; }
@@ -134,6 +134,22 @@ void launch_force_update(int force, const float* m, const float* s, float* r, in
     dim3 grid((nx + 255) / 256, ny, nz);
     if (force == kForceDouble) k_force_update<kForceDouble><<<grid, 256, 0, st>>>(m, s, r, nx, ny, nz, eps_den);
     else k_force_update<kForceSingle><<<grid, 256, 0, st>>>(m, s, r, nx, ny, nz, eps_den);
+}
+
+void launch_force_norms(int force, const float* m, const float* s, const float* r, int nx, int ny, int nz, float eps_den,
+                        StopCtl* ctl, int iter, float stop_eps, int n_sm, cudaStream_t st) {
+    const size_t N = (size_t)nx * ny * nz;
+    size_t blocks = (N + 255) / 256;
+    if (blocks > (size_t)8 * n_sm) blocks = (size_t)8 * n_sm;   // grid-stride: one wave of 8 CTAs per SM
+    if (force == kForceDouble)
+        k_force_norms<kForceDouble><<<(unsigned)blocks, 256, 0, st>>>(m, s, r, nx, ny, nz, eps_den, ctl, iter, stop_eps);
+    else
+        k_force_norms<kForceSingle><<<(unsigned)blocks, 256, 0, st>>>(m, s, r, nx, ny, nz, eps_den, ctl, iter, stop_eps);
+}
+
+void launch_stop_reset(StopCtl* ctl, cudaStream_t st) { k_stop_reset<<<1, 1, 0, st>>>(ctl); }
+void launch_stop_record(StopCtl* ctl, int level, int n_iters, cudaStream_t st) {
+    k_stop_record<<<1, 1, 0, st>>>(ctl, level, n_iters);
 }
 
 void launch_warp_kernel(const float* moving, const float* r, float* out, int nx, int ny, int nz, cudaStream_t st) {

@@ -77,7 +77,8 @@ constexpr int kGzdThreads = 128;
 template <int K, bool WARP, int LZ>
 __global__ void __launch_bounds__(kGzdThreads)
 k_gz_warp_d(const float* __restrict__ rin, float* __restrict__ rout, const float* __restrict__ moving,
-            float* __restrict__ mout, int nx, int ny, int nz, GaussTaps gw) {
+            float* __restrict__ mout, int nx, int ny, int nz, GaussTaps gw, IterCtl ctl) {
+    if (iter_skipped(ctl)) return;
     constexpr int W = 2 * K + 1, NV = LZ + 2 * K;
     const unsigned plane = (unsigned)nx * (unsigned)ny;
     const unsigned col = blockIdx.x * kGzdThreads + threadIdx.x;
@@ -148,7 +149,8 @@ k_gz_warp_d(const float* __restrict__ rin, float* __restrict__ rout, const float
 template <int K, bool WARP, int LZ>
 __global__ void __launch_bounds__(kGzdThreads)
 k_gz_warp_d2(const float* __restrict__ rin, float* __restrict__ rout, const float* __restrict__ moving,
-             float* __restrict__ mout, int nx, int ny, int nz, GaussTaps gw) {
+             float* __restrict__ mout, int nx, int ny, int nz, GaussTaps gw, IterCtl ctl) {
+    if (iter_skipped(ctl)) return;
     constexpr int W = 2 * K + 1, NV = LZ + 2 * K;
     const unsigned plane = (unsigned)nx * (unsigned)ny;
     const unsigned col = 2u * (blockIdx.x * kGzdThreads + threadIdx.x);
@@ -329,7 +331,8 @@ struct FgGroup {
 template <int K, int FORCE>
 __global__ void __launch_bounds__(FgT4Cfg<K>::NT, FgT4Cfg<K>::OCC)
 k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const float* __restrict__ rin,
-               float* __restrict__ rout, int nx, int ny, int nz, float eps_den, GaussTaps gw) {
+               float* __restrict__ rout, int nx, int ny, int nz, float eps_den, GaussTaps gw, IterCtl ctl) {
+    if (iter_skipped(ctl)) return;
     using C = FgT4Cfg<K>;
     constexpr int W = C::W, TX = C::TX, TY = C::TY, NT = C::NT, LX = C::LX, LY = C::LY, PY = C::PY, NG = C::NG;
     constexpr int UP = C::UP, XP = C::XP, KA = C::KA, OFF = C::OFF, NV = C::NV;

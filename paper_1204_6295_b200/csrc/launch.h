@@ -19,6 +19,15 @@ enum MomentsMode {
 };
 
 
+// Stop control handed to every kernel launched from this host thread ({nullptr, 0}: criterion off); set by
+// disc_api.cu around the launches of one iteration.
+extern thread_local IterCtl g_iter_ctl;
+// sum|dr|, sum|r| of the iteration -> l^(k), criterion check in the last block (field.cuh k_force_norms)
+void launch_force_norms(int force, const float* m, const float* s, const float* r, int nx, int ny, int nz, float eps_den,
+                        StopCtl* ctl, int iter, float stop_eps, int n_sm, cudaStream_t st);
+void launch_stop_reset(StopCtl* ctl, cudaStream_t st);
+void launch_stop_record(StopCtl* ctl, int level, int n_iters, cudaStream_t st);
+
 bool launch_moments_any(int R, int mode, int ty, const float* vol, const float* aux, float* out0, float* out1, int nx,
                         int ny, int nz, int zchunk, float eps_var, cudaStream_t st);
 // force = 0 none (plain smoothing), 1 Thirion / passive, 2 double (ForceMode in field.cuh)

@@ -39,7 +39,8 @@ struct MomCfg {
 template <int R, int MODE>
 __global__ void __launch_bounds__(MomCfg<R>::NT, (R <= 6) ? 2 : 1)
 k_moments(const float* __restrict__ vol, const float* __restrict__ aux, float* __restrict__ out0,
-          float* __restrict__ out1, int nx, int ny, int nz, int zchunk, float eps_var) {
+          float* __restrict__ out1, int nx, int ny, int nz, int zchunk, float eps_var, IterCtl ctl) {
+    if (iter_skipped(ctl)) return;
     using C = MomCfg<R>;
     constexpr int W = C::W, PX = C::PX, PY = C::PY, PXP = C::PXP, LX = C::LX, LY = C::LY, XSP = C::XSP;
     constexpr int NT = C::NT, COLS = C::COLS;

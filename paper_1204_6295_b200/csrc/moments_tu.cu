@@ -55,7 +55,7 @@ static bool launch_r_v2(int mode, const float* vol, const float* aux, float* out
             cudaFuncSetAttribute(k_moments_v2<R, TY, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes); \
             configured[M] = true;                                                                                   \
         }                                                                                                           \
-        k_moments_v2<R, TY, M><<<grid, C::NT, C::smem_bytes, st>>>(tmap, tmap_aux, out0, out1, nx, ny, nz, zchunk, eps_var); \
+        k_moments_v2<R, TY, M><<<grid, C::NT, C::smem_bytes, st>>>(tmap, tmap_aux, out0, out1, nx, ny, nz, zchunk, eps_var, g_iter_ctl); \
     }
     if (mode == kModeMoments) DISC_LAUNCH_MODE(kModeMoments)
     else if (mode == kModeZscore) DISC_LAUNCH_MODE(kModeZscore)
@@ -84,11 +84,11 @@ static void launch_r(int mode, int ty, const float* vol, const float* aux, float
     dim3 grid((nx + kMomTX - 1) / kMomTX, (ny + kMomTY - 1) / kMomTY, (nz + zchunk - 1) / zchunk);
     constexpr int NT = MomCfg<R>::NT;
     if (mode == kModeMoments)
-        k_moments<R, kModeMoments><<<grid, NT, 0, st>>>(vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var);
+        k_moments<R, kModeMoments><<<grid, NT, 0, st>>>(vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, g_iter_ctl);
     else if (mode == kModeZscore)
-        k_moments<R, kModeZscore><<<grid, NT, 0, st>>>(vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var);
+        k_moments<R, kModeZscore><<<grid, NT, 0, st>>>(vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, g_iter_ctl);
     else
-        k_moments<R, kModeCorrect><<<grid, NT, 0, st>>>(vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var);
+        k_moments<R, kModeCorrect><<<grid, NT, 0, st>>>(vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, g_iter_ctl);
 }
 
 // one radius: launches if R lies in this unit's range (the discarded branch is never instantiated)

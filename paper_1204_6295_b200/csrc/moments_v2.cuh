@@ -80,7 +80,9 @@ __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.
 template <int R, int TY, int MODE>
 __global__ void __launch_bounds__(MomV2Cfg<R, TY>::NT, TY == 16 ? 2 : 1)
 k_moments_v2(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_aux,
-             float* __restrict__ out0, float* __restrict__ out1, int nx, int ny, int nz, int zchunk, float eps_var) {
+             float* __restrict__ out0, float* __restrict__ out1, int nx, int ny, int nz, int zchunk, float eps_var,
+             IterCtl ctl) {
+    if (iter_skipped(ctl)) return;
     using C = MomV2Cfg<R, TY>;
     constexpr int W = C::W, PY = C::PY, PXB = C::PXB, LX = C::LX, LY = C::LY, XSP = C::XSP;
     constexpr int NP1 = C::NP1, NP2 = C::NP2, NSTG = C::NSTG, NXS = C::NXS, NAUX = C::NAUX, TX = C::TX;

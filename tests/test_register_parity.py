@@ -120,3 +120,51 @@ def test_register_double_force(disc, oracle_mod, dims, R, sigma, levels, iters):
     check(ct, cbct, r, corr, r_ref, corr_ref)
     r1, _ = oracle_mod.register(ct, cbct, R, sigma, levels, iters, want_corr=False)
     assert np.abs(r_ref - r1).max() > 0.05      # and it is a different registration than the Thirion one
+
+
+@pytest.mark.parametrize("dims,R,sigma,levels,iters,eps,double_force", [
+    ((48, 40, 24), 3, 1.5, 2, 40, 2e-3, False),
+    ((64, 64, 32), 3, 1.5, 1, 50, 4e-2, False),      # config 1's schedule with the criterion on (trips at k = 32)
+    ((48, 40, 24), 2, 2.0, 2, 30, 5e-3, True),
+    ((40, 36, 20), 2, 1.5, 2, 14, 1e-4, False),      # the paper's eps: nothing trips, all iterations run
+])
+def test_register_stopping_criterion(disc, oracle_mod, dims, R, sigma, levels, iters, eps, double_force):
+    """NEXT-3: the device-side criterion stops each level where the oracle's does.  The decision
+    compares two floating-point ratios with eps; where the oracle's own margin to eps is below 1e-6 either count is
+    correct, and the field is then checked against the oracle run with the GPU's counts."""
+    ct, cbct, _, _ = phantoms.make_pair(1, dims=dims)
+    nz, ny, nx = ct.shape
+    ctx = disc.disc_create((nx, ny, nz), (1.0, 1.0, 1.0), R, sigma, levels, iters)
+    if double_force:
+        disc.disc_set_force(ctx, disc.DISC_FORCE_DOUBLE)
+    disc.disc_set_stop(ctx, eps)
+    d_r = torch.empty((3,) + ct.shape, device="cuda")
+    d_c = torch.empty(ct.shape, device="cuda")
+    disc.disc_register(ctx, dev(ct), dev(cbct), d_r, d_c)
+    run = np.array(disc.disc_iterations_run(ctx))
+    r_ref, run_ref, lt = oracle_mod.register_stop(ct, cbct, R, sigma, levels, iters, stop_eps=eps, double_force=double_force)
+    if not np.array_equal(run, run_ref):
+        for lev in range(levels):
+            if run[lev] != run_ref[lev]:
+                k = min(run[lev], run_ref[lev]) - 1            # the iteration where the two decisions differ
+                row = lt[levels - 1 - lev]
+                assert k >= 10 and abs(row[k - 10] - row[k] - eps) < 1e-6, (lev, run, run_ref)
+                break                                           # later levels start from different fields
+        r_ref, _, _ = oracle_mod.register_stop(ct, cbct, R, sigma, levels, iters, iters_per_level=run, double_force=double_force)
+    assert np.abs(d_r.cpu().numpy() - r_ref).max() <= 1e-2
+    if eps > 1e-4:
+        assert run.min() < iters                                # the case is meant to stop early somewhere
+    else:
+        assert np.all(run == iters)
+    # reading A12 still holds after an early stop: the returned corrected CBCT belongs to the returned field
+    d_m, d_c2 = torch.empty_like(d_c), torch.empty_like(d_c)
+    disc.disc_warp(ctx, 0, dev(ct), d_r, d_m)
+    disc.disc_correct_intensity(ctx, 0, dev(cbct), d_m, d_c2)
+    assert torch.equal(d_c2, d_c)
+    # switching the criterion off restores the fixed schedule
+    disc.disc_set_stop(ctx, -1.0)
+    disc.disc_register(ctx, dev(ct), dev(cbct), d_r, d_c)
+    assert disc.disc_iterations_run(ctx) == [iters] * levels
+    r_fix, _ = oracle_mod.register(ct, cbct, R, sigma, levels, iters, want_corr=False, double_force=double_force)
+    assert np.abs(d_r.cpu().numpy() - r_fix).max() <= 1e-2
+    disc.disc_destroy(ctx)
