@@ -234,6 +234,9 @@ k_gz_warp_d2(const float* __restrict__ rin, float* __restrict__ rout, const floa
 // the replicate border: the clamped point's value, broadcast.
 // Requirements (launcher): nx % 4 == 0, 16-byte aligned m, s, rin, rout.
 // ---------------------------------------------------------------------------------------------------------
+#ifndef DISC_FG_LX
+#define DISC_FG_LX 8
+#endif
 #ifndef DISC_FG_TY
 #define DISC_FG_TY 32
 #endif
@@ -245,7 +248,7 @@ k_gz_warp_d2(const float* __restrict__ rin, float* __restrict__ rout, const floa
 #endif
 template <int K>
 struct FgT4Cfg {
-    static constexpr int TX = 64, TY = DISC_FG_TY, NT = DISC_FG_NT, OCC = DISC_FG_OCC, LX = 8, LY = 8;
+    static constexpr int TX = 64, TY = DISC_FG_TY, NT = DISC_FG_NT, OCC = DISC_FG_OCC, LX = DISC_FG_LX, LY = 8;
     static constexpr int W = 2 * K + 1;
     static constexpr int KA = (K + 3) / 4 * 4, OFF = KA - K;
     static constexpr int PXA = TX + 2 * KA, PY = TY + 2 * K, NG = PXA / 4;
@@ -426,8 +429,8 @@ k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const f
                 o[j] = acc;
             }
             float4* xp = reinterpret_cast<float4*>(X + (cc * PY + r) * XP + g * LX);
-            xp[0] = make_float4(o[0], o[1], o[2], o[3]);
-            xp[1] = make_float4(o[4], o[5], o[6], o[7]);
+#pragma unroll
+            for (int q4 = 0; q4 < LX / 4; ++q4) xp[q4] = make_float4(o[4 * q4], o[4 * q4 + 1], o[4 * q4 + 2], o[4 * q4 + 3]);
         }
         __syncthreads();
         px0 = x0; py0 = y0; pz = z; have_prev = true;
