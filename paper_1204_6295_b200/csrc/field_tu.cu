@@ -16,7 +16,8 @@ static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t
 template <int K, int FORCE>
 static void launch_fg(int txb, const float* m, const float* s, const float* rin, float* rout, int nx, int ny, int nz,
                       int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
-    const bool vec_ok = nx % 4 == 0 && aligned16(rin) && aligned16(rout) && (!FORCE || (aligned16(m) && aligned16(s)));
+    const bool vec_ok = nx % 4 == 0 && aligned16(rin) && aligned16(rout) && (!FORCE || (aligned16(m) && aligned16(s))) &&
+                        3ull * nx * ny * nz < 0xffffffffull;   // the tile kernel indexes voxels with 32 bits
     static int n_sm = 0;
     if (!n_sm) {
         int dev = 0;

@@ -263,7 +263,18 @@ struct FgT4Cfg {
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 
-// updated field of one group of four x-adjacent points (gx % 4 == 0), loads first, arithmetic after
+__device__ __forceinline__ float rcp_approx(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// updated field of one group of four x-adjacent points (gx % 4 == 0), loads first, arithmetic after.
+// Voxel indices are 32-bit here (the launcher checks 3 N < 2^32): one IMAD.WIDE per load instead of a 64-bit add.
+// The force is evaluated with the raw central differences D = 2 g and t = 2 d:
+//   d g_c / (|g|^2 + d^2 + eps) = (t / (|D|^2 + t^2 + 4 eps)) * D_c
+// -- the same real number (every scaling is by a power of two, so the fused chains round identically) without the
+// twelve multiplications by 1/2; the quotient is t * rcp.approx(den), den >= 4 eps > 0.
 template <int FORCE>
 struct FgGroup {
     float4 u[3], sc, mm, syp, sym, szp, szm;
@@ -271,20 +282,23 @@ struct FgGroup {
     float4 myp, mym, mzp, mzm;   // double force only: the moving image's neighbours
     float ml, mr;
     __device__ __forceinline__ void load(const float* __restrict__ m, const float* __restrict__ s,
-                                         const float* __restrict__ rin, int nx, int ny, int nz, size_t plane, size_t N,
+                                         const float* __restrict__ rin, int nx, int ny, int nz, unsigned plane, unsigned N,
                                          int gx, int gy, int z) {
-        const size_t i = (size_t)z * plane + (size_t)gy * nx + gx;
+        const unsigned i = (unsigned)z * plane + (unsigned)gy * (unsigned)nx + (unsigned)gx;
 #pragma unroll
-        for (int c = 0; c < 3; ++c) u[c] = ldg4(rin + c * N + i);
+        for (int c = 0; c < 3; ++c) u[c] = ldg4(rin + (i + (unsigned)c * N));
         if (FORCE) {
+            const unsigned il = i - (gx > 0 ? 1u : 0u), ir = i + 3u + (gx + 4 < nx ? 1u : 0u);
+            const unsigned iyp = i + (gy < ny - 1 ? (unsigned)nx : 0u), iym = i - (gy > 0 ? (unsigned)nx : 0u);
+            const unsigned izp = i + (z < nz - 1 ? plane : 0u), izm = i - (z > 0 ? plane : 0u);
             sc = ldg4(s + i); mm = ldg4(m + i);
-            sl = __ldg(s + i - (gx > 0 ? 1 : 0)); sr = __ldg(s + i + 3 + (gx + 4 < nx ? 1 : 0));
-            syp = ldg4(s + i + (gy < ny - 1 ? (size_t)nx : 0)); sym = ldg4(s + i - (gy > 0 ? (size_t)nx : 0));
-            szp = ldg4(s + i + (z < nz - 1 ? plane : 0)); szm = ldg4(s + i - (z > 0 ? plane : 0));
+            sl = __ldg(s + il); sr = __ldg(s + ir);
+            syp = ldg4(s + iyp); sym = ldg4(s + iym);
+            szp = ldg4(s + izp); szm = ldg4(s + izm);
             if (FORCE == kForceDouble) {
-                ml = __ldg(m + i - (gx > 0 ? 1 : 0)); mr = __ldg(m + i + 3 + (gx + 4 < nx ? 1 : 0));
-                myp = ldg4(m + i + (gy < ny - 1 ? (size_t)nx : 0)); mym = ldg4(m + i - (gy > 0 ? (size_t)nx : 0));
-                mzp = ldg4(m + i + (z < nz - 1 ? plane : 0)); mzm = ldg4(m + i - (z > 0 ? plane : 0));
+                ml = __ldg(m + il); mr = __ldg(m + ir);
+                myp = ldg4(m + iyp); mym = ldg4(m + iym);
+                mzp = ldg4(m + izp); mzm = ldg4(m + izm);
             }
         }
     }
@@ -299,25 +313,23 @@ struct FgGroup {
             const float he[6] = {ml, mm.x, mm.y, mm.z, mm.w, mr};
             const float hyp[4] = {myp.x, myp.y, myp.z, myp.w}, hym[4] = {mym.x, mym.y, mym.z, mym.w};
             const float hzp[4] = {mzp.x, mzp.y, mzp.z, mzp.w}, hzm[4] = {mzm.x, mzm.y, mzm.z, mzm.w};
+            const float eps4 = 4.f * eps_den;
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
-                const float gxv = 0.5f * (ce[e + 2] - ce[e]);
-                const float gyv = 0.5f * (yp[e] - ym[e]);
-                const float gzv = 0.5f * (zp[e] - zm[e]);
+                const float Dx = ce[e + 2] - ce[e], Dy = yp[e] - ym[e], Dz = zp[e] - zm[e];
                 const float d = ce[e + 1] - me[e];
-                const float dd = fmaf(d, d, eps_den);
-                const float q = __fdividef(d, fmaf(gxv, gxv, fmaf(gyv, gyv, fmaf(gzv, gzv, dd))));
-                ux[e] = fmaf(q, gxv, ux[e]);
-                uy[e] = fmaf(q, gyv, uy[e]);
-                uz[e] = fmaf(q, gzv, uz[e]);
+                const float t = d + d;
+                const float tt = fmaf(t, t, eps4);
+                const float q = t * rcp_approx(fmaf(Dx, Dx, fmaf(Dy, Dy, fmaf(Dz, Dz, tt))));
+                ux[e] = fmaf(q, Dx, ux[e]);
+                uy[e] = fmaf(q, Dy, uy[e]);
+                uz[e] = fmaf(q, Dz, uz[e]);
                 if (FORCE == kForceDouble) {
-                    const float hxv = 0.5f * (he[e + 2] - he[e]);
-                    const float hyv = 0.5f * (hyp[e] - hym[e]);
-                    const float hzv = 0.5f * (hzp[e] - hzm[e]);
-                    const float p = __fdividef(d, fmaf(hxv, hxv, fmaf(hyv, hyv, fmaf(hzv, hzv, dd))));
-                    ux[e] = fmaf(p, hxv, ux[e]);
-                    uy[e] = fmaf(p, hyv, uy[e]);
-                    uz[e] = fmaf(p, hzv, uz[e]);
+                    const float Hx = he[e + 2] - he[e], Hy = hyp[e] - hym[e], Hz = hzp[e] - hzm[e];
+                    const float p = t * rcp_approx(fmaf(Hx, Hx, fmaf(Hy, Hy, fmaf(Hz, Hz, tt))));
+                    ux[e] = fmaf(p, Hx, ux[e]);
+                    uy[e] = fmaf(p, Hy, uy[e]);
+                    uz[e] = fmaf(p, Hz, uz[e]);
                 }
             }
             u[0] = make_float4(ux[0], ux[1], ux[2], ux[3]);
@@ -364,15 +376,17 @@ k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const f
                 const int gx = x0 - KA + 4 * g;
                 // a group wholly outside the volume is the replicate border: the edge group's outermost value
                 FgGroup<FORCE> G;
-                G.load(m, s, rin, nx, ny, nz, plane, N, clampi(gx, 0, nx - 4), gy, z);
+                G.load(m, s, rin, nx, ny, nz, (unsigned)plane, (unsigned)N, clampi(gx, 0, nx - 4), gy, z);
                 G.finish(eps_den);
+                if (gx < 0 || gx >= nx) {   // only in the tiles at the volume's x border
 #pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    float4 v = G.u[c];
-                    if (gx < 0) v = make_float4(v.x, v.x, v.x, v.x);
-                    else if (gx >= nx) v = make_float4(v.w, v.w, v.w, v.w);
-                    *reinterpret_cast<float4*>(U + (c * PY + r) * UP + 4 * g) = v;
+                    for (int c = 0; c < 3; ++c) {
+                        const float e = gx < 0 ? G.u[c].x : G.u[c].w;
+                        G.u[c] = make_float4(e, e, e, e);
+                    }
                 }
+#pragma unroll
+                for (int c = 0; c < 3; ++c) *reinterpret_cast<float4*>(U + (c * PY + r) * UP + 4 * g) = G.u[c];
             }
         }
         // ---- phase 3 of tile t-1: y pass, lanes <-> column groups
@@ -400,10 +414,18 @@ k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const f
                 const int gx = px0 + cg * 4;
                 if (gx < nx) {
                     float* op = rout + cc * N + ((size_t)pz * ny + (py0 + h * LY)) * nx + gx;
+                    if (py0 + h * LY + LY <= ny) {   // whole run inside the volume: no per-row test
 #pragma unroll
-                    for (int j = 0; j < LY; ++j)
-                        if (py0 + h * LY + j < ny)
-                            *reinterpret_cast<float4*>(op + (size_t)j * nx) = make_float4(a0[j].x, a0[j].y, a1[j].x, a1[j].y);
+                        for (int j = 0; j < LY; ++j) {
+                            *reinterpret_cast<float4*>(op) = make_float4(a0[j].x, a0[j].y, a1[j].x, a1[j].y);
+                            op += nx;
+                        }
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < LY; ++j)
+                            if (py0 + h * LY + j < ny)
+                                *reinterpret_cast<float4*>(op + (size_t)j * nx) = make_float4(a0[j].x, a0[j].y, a1[j].x, a1[j].y);
+                    }
                 }
             }
         }
