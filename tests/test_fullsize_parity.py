@@ -161,3 +161,35 @@ def test_config4_finest_level_sampled(disc, oracle_mod):
     disc.disc_warp(ctx, 0, d_a, d_u, d_m)
     assert np.abs(d_m.cpu().numpy() - oracle_mod.warp(a, u)).max() <= 1e-4 * span
     disc.disc_destroy(ctx)
+
+
+@pytest.mark.slow
+def test_config4_whole_schedule_properties(disc, oracle_mod):
+    """config 4 as BASELINE.json states it: 512x512x128, 4-level pyramid x 100 iterations, patch 15^3 (R = 7), sigma 2.
+    The naive oracle would need over an hour for this schedule, so the whole run is checked through properties that
+    hold at any size and through the oracle at sampled voxels of the returned corrected CBCT."""
+    ct, cbct, u, p = phantoms.make_pair(4)
+    nz, ny, nx = ct.shape
+    assert (nx, ny, nz) == (512, 512, 128) and p["patch_radius"] == 7 and p["levels"] == 4
+    R, sigma = p["patch_radius"], p["sigma"]
+    ctx = disc.disc_create((nx, ny, nz), (1, 1, 1), R, sigma, p["levels"], p["iters"])
+    d_ct, d_cb = dev(ct), dev(cbct)
+    d_r, d_corr = torch.empty((3,) + ct.shape, device="cuda"), torch.empty_like(d_ct)
+    disc.disc_register(ctx, d_ct, d_cb, d_r, d_corr)
+    assert disc.disc_iterations_run(ctx) == [p["iters"]] * p["levels"]
+    d_m, d_c2 = torch.empty_like(d_ct), torch.empty_like(d_ct)
+    disc.disc_warp(ctx, 0, d_ct, d_r, d_m)
+    disc.disc_correct_intensity(ctx, 0, d_cb, d_m, d_c2)
+    assert torch.equal(d_c2, d_corr)                                   # reading A12
+    assert bool(torch.isfinite(d_r).all())
+    m = d_m.cpu().numpy()
+    idx = sample_indices(ct.shape, np.random.default_rng(17), 120)
+    span = hu_range(ct, cbct)
+    assert np.abs(d_corr.cpu().numpy().ravel()[idx] - oracle_mod.correct_at(cbct, m, R, idx)).max() <= 1e-4 * span
+    assert np.abs(m - oracle_mod.warp(ct, d_r.cpu().numpy())).max() <= 1e-4 * span
+    target = phantoms.pullback(ct, u)
+    body = target > -500.0
+    rmse0 = np.sqrt(np.mean((ct - target)[body] ** 2))
+    rmse1 = np.sqrt(np.mean((m - target)[body] ** 2))
+    assert rmse1 < 0.7 * rmse0, (rmse0, rmse1)
+    disc.disc_destroy(ctx)
