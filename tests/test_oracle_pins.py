@@ -70,6 +70,30 @@ def test_P3_moments_ramp_closed_form(oracle_mod, R):
     np.testing.assert_allclose(var[c, c, c], expect, rtol=1e-12)
 
 
+def test_golden_ramp_variance_and_paper_constants(oracle_mod):
+    """tests/golden: the closed-form ramp variance table (Eq. 3) and the constants the paper prints."""
+    import os
+    gdir = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    rows = [ln.split() for ln in open(os.path.join(gdir, "ramp_variance.txt")) if ln.strip() and not ln.startswith("#")]
+    g = (3.0, -2.0, 0.5)                                   # slopes along x, y, z
+    n = 25
+    z, y, x = np.meshgrid(np.arange(float(n)), np.arange(float(n)), np.arange(float(n)), indexing="ij")
+    vol = (g[0] * x + g[1] * y + g[2] * z).astype(np.float32)
+    c = n // 2
+    for R_s, v_s in rows:
+        R, per_unit = int(R_s), float(v_s)
+        mean, var = oracle_mod.box_moments(vol, R)
+        np.testing.assert_allclose(var[c, c, c], per_unit * sum(t * t for t in g), rtol=1e-9, atol=1e-9)
+        np.testing.assert_allclose(mean[c, c, c], vol[c, c, c], rtol=1e-12)
+    consts = {ln.split()[0]: ln.split()[1] for ln in open(os.path.join(gdir, "paper_constants.txt"))
+              if ln.strip() and not ln.startswith("#")}
+    assert float(consts["stop_eps"]) == 1.0e-4 and int(consts["stop_lag"]) == 10
+    # the oracle's criterion uses exactly that lag: with eps = +inf it trips at k = 10, i.e. after 11 iterations
+    ct, cbct, _, _ = phantoms.make_pair(1, dims=(24, 20, 12))
+    _, run, _ = oracle_mod.register_stop(ct, cbct, 1, 1.0, 1, 20, stop_eps=float("inf"))
+    assert int(run[0]) == int(consts["stop_lag"]) + 1
+
+
 def test_P4_moments_scipy_uniform_filter(oracle_mod):
     rng = np.random.default_rng(4)
     v = rng.normal(0, 100, size=(12, 11, 13)).astype(np.float32)
