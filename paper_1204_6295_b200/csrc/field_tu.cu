@@ -154,6 +154,11 @@ void launch_stop_record(StopCtl* ctl, int level, int n_iters, cudaStream_t st) {
 }
 
 void launch_warp_kernel(const float* moving, const float* r, float* out, int nx, int ny, int nz, cudaStream_t st) {
+    if (nx % 2 == 0 && (reinterpret_cast<uintptr_t>(r) & 7u) == 0 && (reinterpret_cast<uintptr_t>(out) & 7u) == 0) {
+        dim3 grid2((nx / 2 + 127) / 128, ny, nz);
+        k_warp2<<<grid2, 128, 0, st>>>(moving, r, out, nx, ny, nz);
+        return;
+    }
     dim3 grid((nx + 255) / 256, ny, nz);
     k_warp<<<grid, 256, 0, st>>>(moving, r, out, nx, ny, nz);
 }

@@ -72,6 +72,30 @@ __device__ __forceinline__ float tri_finish(const TriSample& s) {
     return fmaf(s.tz, c1, uz * c0);
 }
 
+// Step (b) alone (disc_warp) with two x-adjacent voxels per thread: 8-byte field loads and stores, both samples'
+// sixteen gathered loads issued before either is interpolated.  Needs nx even and 8-byte aligned r, out.
+static __global__ void __launch_bounds__(128)
+k_warp2(const float* __restrict__ moving, const float* __restrict__ r, float* __restrict__ out, int nx, int ny, int nz) {
+    const int x = 2 * (blockIdx.x * blockDim.x + threadIdx.x);
+    const int y = blockIdx.y, z = blockIdx.z;
+    if (x >= nx) return;
+    const size_t N = (size_t)nx * ny * nz;
+    const size_t i = ((size_t)z * ny + y) * nx + x;
+    const float2 rx = __ldg(reinterpret_cast<const float2*>(r + i));
+    const float2 ry = __ldg(reinterpret_cast<const float2*>(r + N + i));
+    const float2 rz = __ldg(reinterpret_cast<const float2*>(r + 2 * N + i));
+    const bool fast = nx > 1 && ny > 1 && nz > 1 && N < (size_t)0x7fffffff;   // 32-bit voxel indices
+    TriSample g0, g1;
+    if (fast) {
+        tri_issue<true>(moving, nx, ny, nz, (float)x + rx.x, (float)y + ry.x, (float)z + rz.x, g0);
+        tri_issue<true>(moving, nx, ny, nz, (float)(x + 1) + rx.y, (float)y + ry.y, (float)z + rz.y, g1);
+    } else {
+        tri_issue<false>(moving, nx, ny, nz, (float)x + rx.x, (float)y + ry.x, (float)z + rz.x, g0);
+        tri_issue<false>(moving, nx, ny, nz, (float)(x + 1) + rx.y, (float)y + ry.y, (float)z + rz.y, g1);
+    }
+    *reinterpret_cast<float2*>(out + i) = make_float2(tri_finish(g0), tri_finish(g1));
+}
+
 constexpr int kGzdThreads = 128;
 
 template <int K, bool WARP, int LZ>
