@@ -168,3 +168,22 @@ def test_register_stopping_criterion(disc, oracle_mod, dims, R, sigma, levels, i
     r_fix, _ = oracle_mod.register(ct, cbct, R, sigma, levels, iters, want_corr=False, double_force=double_force)
     assert np.abs(d_r.cpu().numpy() - r_fix).max() <= 1e-2
     disc.disc_destroy(ctx)
+
+
+def test_register_degenerate_schedules(disc, oracle_mod):
+    """edge cases of the driver: zero iterations (the field stays zero, the corrected CBCT is correct(cbct, ct)), a
+    one-voxel-thick volume, and a volume with a single column"""
+    ct, cbct, _, _ = phantoms.make_pair(1, dims=(32, 24, 16))
+    r, corr, n = gpu_register(disc, ct, cbct, 2, 1.5, 2, 0)
+    assert not r.any()
+    span = float(max(ct.max(), cbct.max()) - min(ct.min(), cbct.min()))
+    assert np.abs(corr - oracle_mod.correct(cbct, ct, 2)).max() <= 1e-4 * span
+    for dims in ((20, 18, 1), (1, 1, 24), (4, 1, 6)):
+        ct2, cbct2, _, _ = phantoms.make_pair(1, dims=dims)
+        r, corr, _ = gpu_register(disc, ct2, cbct2, 1, 1.0, 1, 6)
+        r_ref, corr_ref = oracle_mod.register(ct2, cbct2, 1, 1.0, 1, 6)
+        err_r = np.abs(r - r_ref).max()
+        assert err_r <= 1e-2, (dims, err_r)
+        span = float(max(ct2.max(), cbct2.max()) - min(ct2.min(), cbct2.min()))
+        steep = max([np.abs(np.diff(ct2.astype(np.float64), axis=a)).max() for a in range(3) if ct2.shape[a] > 1] + [0.0])
+        assert np.abs(corr - corr_ref).max() <= 1e-4 * span + 2.0 * err_r * steep + 1e-3, dims
