@@ -230,3 +230,176 @@ def register_stop(ct, cbct, R, sigma, levels, iters, stop_eps=None, iters_per_le
                            ipl.ctypes.data_as(i32p) if ipl is not None else None, run.ctypes.data_as(i32p),
                            ltrace.ctypes.data_as(_f64p), disp.ctypes.data_as(_f32p), None, None)
     return disp, run, ltrace
+
+
+# ------------------------------------------------------------------------------------------------
+# SURVEY.md section 8(f) extensions: NEXT-4 (per-axis patch radius, per-axis pyramid factor), NEXT-1 (mask and
+# interpolation of a, b), Fig.-9 diagnostics, summed-area moments.
+# ------------------------------------------------------------------------------------------------
+_i32p = ctypes.POINTER(ctypes.c_int)
+_u8p = ctypes.POINTER(ctypes.c_ubyte)
+
+
+def _r3(R):
+    """patch radius as (Rx, Ry, Rz): an int means the cube of the hot path"""
+    r = (R, R, R) if np.isscalar(R) else tuple(int(v) for v in R)
+    assert len(r) == 3
+    return (ctypes.c_int * 3)(*r)
+
+
+def box_moments3(vol, R, sat=False):
+    """(mean, var) over the truncated box of per-axis radius R = (Rx, Ry, Rz); sat=True uses the
+    independently written fp64 summed-area routine."""
+    L = _load()
+    v, pv = _f32(vol)
+    mean = np.empty(v.shape, dtype=np.float64)
+    var = np.empty(v.shape, dtype=np.float64)
+    fn = L.oracle_box_moments_sat if sat else L.oracle_box_moments3
+    fn(pv, *_dims(v), _r3(R), mean.ctypes.data_as(_f64p), var.ctypes.data_as(_f64p))
+    return mean, var
+
+
+def correct3(cbct, ct_warped, R, eps_var=EPS_VAR):
+    """correct() with a per-axis patch radius."""
+    mus, vs = box_moments3(cbct, R)
+    mum, vm = box_moments3(ct_warped, R)
+    return correct_from_moments(cbct, mus, vs, mum, vm, eps_var)
+
+
+def downsample3(vol, fac):
+    """block mean over fac = (fx, fy, fz) voxels, each factor 1 or 2."""
+    L = _load()
+    v, pv = _f32(vol)
+    nz, ny, nx = v.shape
+    out = np.empty((nz // fac[2], ny // fac[1], nx // fac[0]), dtype=np.float32)
+    L.oracle_downsample3(pv, *_dims(v), (ctypes.c_int * 3)(*fac), out.ctypes.data_as(_f32p))
+    return out
+
+
+def upsample_field3(disp, fac):
+    """field up-sampling with a per-axis factor (reading A9)."""
+    L = _load()
+    d, pd = _f32(disp)
+    _, nz, ny, nx = d.shape
+    out = np.empty((3, fac[2] * nz, fac[1] * ny, fac[0] * nx), dtype=np.float32)
+    L.oracle_upsample_field3(pd, ctypes.c_int(nx), ctypes.c_int(ny), ctypes.c_int(nz), (ctypes.c_int * 3)(*fac),
+                             out.ctypes.data_as(_f32p))
+    return out
+
+
+def ab_from_moments(mu_s, var_s, mu_m, var_m, eps_var=EPS_VAR):
+    """Eqs. (5), (6): a = STD(M)/STD(S), b = E(M) - a E(S)."""
+    L = _load()
+    arrs = [np.ascontiguousarray(x, dtype=np.float64) for x in (mu_s, var_s, mu_m, var_m)]
+    a = np.empty(arrs[0].shape, dtype=np.float64)
+    b = np.empty(arrs[0].shape, dtype=np.float64)
+    L.oracle_ab_from_moments(*[x.ctypes.data_as(_f64p) for x in arrs], ctypes.c_size_t(a.size), ctypes.c_double(eps_var),
+                             a.ctypes.data_as(_f64p), b.ctypes.data_as(_f64p))
+    return a, b
+
+
+def mask(m, cbct, a, hu0, a_min, a_max):
+    """Eq. (7): xi = 1 where |I_m - I_s| > HU_0 or a outside [a_min, a_max]."""
+    L = _load()
+    m_, pm = _f32(m)
+    s_, ps = _f32(cbct)
+    a_ = np.ascontiguousarray(a, dtype=np.float64)
+    xi = np.empty(m_.shape, dtype=np.uint8)
+    L.oracle_mask(pm, ps, a_.ctypes.data_as(_f64p), ctypes.c_size_t(m_.size), ctypes.c_double(hu0), ctypes.c_double(a_min),
+                  ctypes.c_double(a_max), xi.ctypes.data_as(_u8p))
+    return xi
+
+
+def fill_ab(cbct, xi, a, b, fill_radius, h, max_passes=64):
+    """Eqs. (8)-(10): interpolate / extrapolate a, b into the xi = 1 voxels.  Returns
+    (a, b, xi_left, passes)."""
+    L = _load()
+    s_, ps = _f32(cbct)
+    x = np.array(xi, dtype=np.uint8, order="C", copy=True)
+    a_ = np.array(a, dtype=np.float64, order="C", copy=True)
+    b_ = np.array(b, dtype=np.float64, order="C", copy=True)
+    L.oracle_fill_ab.restype = ctypes.c_int
+    n = L.oracle_fill_ab(ps, *_dims(s_), x.ctypes.data_as(_u8p), a_.ctypes.data_as(_f64p), b_.ctypes.data_as(_f64p),
+                         ctypes.c_int(fill_radius), ctypes.c_double(h), ctypes.c_int(max_passes))
+    return a_, b_, x, int(n)
+
+
+def apply_ab(cbct, a, b):
+    """I'_s = a I_s + b."""
+    L = _load()
+    s_, ps = _f32(cbct)
+    a_ = np.ascontiguousarray(a, dtype=np.float64)
+    b_ = np.ascontiguousarray(b, dtype=np.float64)
+    out = np.empty_like(s_)
+    L.oracle_apply_ab(ps, a_.ctypes.data_as(_f64p), b_.ctypes.data_as(_f64p), ctypes.c_size_t(s_.size),
+                      out.ctypes.data_as(_f32p))
+    return out
+
+
+def delta_hu(ct, cbct):
+    """Delta HU = mean(CT) - mean(CBCT)."""
+    L = _load()
+    a, pa = _f32(ct)
+    b, pb = _f32(cbct)
+    L.oracle_delta_hu.restype = ctypes.c_double
+    return float(L.oracle_delta_hu(pa, pb, ctypes.c_size_t(a.size)))
+
+
+def median_a(a, var_s, var_m, eps_var=EPS_VAR):
+    """a_m = median(A) before the DIR (reading A17)."""
+    L = _load()
+    arrs = [np.ascontiguousarray(x, dtype=np.float64) for x in (a, var_s, var_m)]
+    L.oracle_median_a.restype = ctypes.c_double
+    return float(L.oracle_median_a(*[x.ctypes.data_as(_f64p) for x in arrs], ctypes.c_size_t(arrs[0].size),
+                                   ctypes.c_double(eps_var)))
+
+
+class _Params(ctypes.Structure):
+    _fields_ = [("R", ctypes.c_int * 3), ("fac", ctypes.c_int * 3), ("sigma", ctypes.c_double),
+                ("levels", ctypes.c_int), ("iters", ctypes.c_int), ("eps_var", ctypes.c_double),
+                ("eps_den", ctypes.c_double), ("double_force", ctypes.c_int), ("stop_eps", ctypes.c_double),
+                ("moments_policy", ctypes.c_int), ("mask", ctypes.c_int), ("hu0", ctypes.c_double),
+                ("a_min", ctypes.c_double), ("a_max", ctypes.c_double), ("fill_radius", ctypes.c_int),
+                ("h", ctypes.c_double), ("max_fill_passes", ctypes.c_int)]
+
+
+class _Info(ctypes.Structure):
+    _fields_ = [("delta_hu", ctypes.c_double), ("hu0", ctypes.c_double), ("a_m", ctypes.c_double),
+                ("a_min", ctypes.c_double), ("a_max", ctypes.c_double)]
+
+
+def register_ex(ct, cbct, R, sigma, levels, iters, fac=(2, 2, 2), double_force=False, stop_eps=None, sat_between=False,
+                mask=False, hu0=None, a_range=None, fill_radius=1, h=50.0, max_fill_passes=64, want_corr=True,
+                eps_var=EPS_VAR, eps_den=EPS_DEN):
+    """Algorithm A1 with every option of the oracle: per-axis patch radius R and pyramid factor
+    `fac` (NEXT-4), double force (NEXT-2), stopping criterion (NEXT-3), mask + interpolation of a, b with the global
+    Delta-HU shift (NEXT-1), and `sat_between` = summed-area moments in all but the first and last iteration of a
+    level (config 4's whole-schedule check).  Returns a dict: disp, corr, iters_run [levels, 0 = finest], l, mean_a,
+    mean_b [levels, iters] (coarsest level first, nan where not run), info."""
+    L = _load()
+    a, pa = _f32(ct)
+    b, pb = _f32(cbct)
+    prm = _Params()
+    prm.R = _r3(R)
+    prm.fac = (ctypes.c_int * 3)(*fac)
+    prm.sigma, prm.levels, prm.iters = float(sigma), int(levels), int(iters)
+    prm.eps_var, prm.eps_den = float(eps_var), float(eps_den)
+    prm.double_force = 1 if double_force else 0
+    prm.stop_eps = -1.0 if stop_eps is None else float(stop_eps)
+    prm.moments_policy = 1 if sat_between else 0
+    prm.mask = 1 if mask else 0
+    prm.hu0 = -1.0 if hu0 is None else float(hu0)
+    prm.a_min, prm.a_max = (-1.0, -1.0) if a_range is None else (float(a_range[0]), float(a_range[1]))
+    prm.fill_radius, prm.h, prm.max_fill_passes = int(fill_radius), float(h), int(max_fill_passes)
+    disp = np.empty((3,) + a.shape, dtype=np.float32)
+    corr = np.empty_like(a) if want_corr else None
+    run = np.zeros(levels, dtype=np.int32)
+    shape = (levels, max(iters, 1))
+    ltrace, mean_a, mean_b = (np.full(shape, np.nan, dtype=np.float64) for _ in range(3))
+    info = _Info()
+    L.oracle_register_ex(pa, pb, *_dims(a), ctypes.byref(prm), disp.ctypes.data_as(_f32p),
+                         corr.ctypes.data_as(_f32p) if want_corr else None, run.ctypes.data_as(_i32p),
+                         ltrace.ctypes.data_as(_f64p), mean_a.ctypes.data_as(_f64p), mean_b.ctypes.data_as(_f64p),
+                         ctypes.byref(info))
+    return {"disp": disp, "corr": corr, "iters_run": run, "l": ltrace, "mean_a": mean_a, "mean_b": mean_b,
+            "info": {k: getattr(info, k) for k, _ in _Info._fields_}}

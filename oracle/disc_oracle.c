@@ -17,10 +17,11 @@
  * Patch loops are naive (every voxel visits its whole patch, as the paper's own
  * kernel does); variance is two-pass.  OpenMP over z only.
  *
- * Every function is pinned by tests/test_oracle_pins.py (closed forms,
- * invariants, brute force, scipy special cases) -- no function is "parity
- * unpinned" except registration accuracy on the paper's clinical data
- * (PAPER.md:347-378), which is not reproducible here and not claimed.
+ * Every function is pinned by tests/test_oracle_pins.py and
+ * tests/test_oracle_pins_ext.py (closed forms, invariants, brute force, hand
+ * values, scipy special cases) -- no function is "parity unpinned" except
+ * registration accuracy on the paper's clinical data, which
+ * is not reproducible here and not claimed.
  */
 #include <math.h>
 #include <stdlib.h>
@@ -87,11 +88,11 @@ void oracle_warp(const float *I, const float *disp, int nx, int ny, int nz, floa
  * volume (reading A4): n(x) = number of in-volume voxels.  Two-pass variance
  * sum (x - mu)^2 / n, which equals E(X^2) - E(X)^2 in exact arithmetic.
  * ---------------------------------------------------------------------- */
-static inline void patch_stats(const float *v, int nx, int ny, int nz, int R, int x, int y, int z,
-                               double *mean, double *var) {
-    int x0 = x - R < 0 ? 0 : x - R, x1 = x + R > nx - 1 ? nx - 1 : x + R;
-    int y0 = y - R < 0 ? 0 : y - R, y1 = y + R > ny - 1 ? ny - 1 : y + R;
-    int z0 = z - R < 0 ? 0 : z - R, z1 = z + R > nz - 1 ? nz - 1 : z + R;
+static inline void patch_stats3(const float *v, int nx, int ny, int nz, const int R[3], int x, int y, int z,
+                                double *mean, double *var) {
+    int x0 = x - R[0] < 0 ? 0 : x - R[0], x1 = x + R[0] > nx - 1 ? nx - 1 : x + R[0];
+    int y0 = y - R[1] < 0 ? 0 : y - R[1], y1 = y + R[1] > ny - 1 ? ny - 1 : y + R[1];
+    int z0 = z - R[2] < 0 ? 0 : z - R[2], z1 = z + R[2] > nz - 1 ? nz - 1 : z + R[2];
     double n = (double)(x1 - x0 + 1) * (y1 - y0 + 1) * (z1 - z0 + 1);
     double s = 0.0;
     for (int c = z0; c <= z1; ++c)
@@ -102,6 +103,13 @@ static inline void patch_stats(const float *v, int nx, int ny, int nz, int R, in
         for (int b = y0; b <= y1; ++b)
             for (int a = x0; a <= x1; ++a) { double d = v[IDX(a, b, c)] - mu; q += d * d; }
     *mean = mu; *var = q / n;
+}
+
+/* the cubic patch of the hot path: the same radius on every axis */
+static inline void patch_stats(const float *v, int nx, int ny, int nz, int R, int x, int y, int z,
+                               double *mean, double *var) {
+    const int R3[3] = {R, R, R};
+    patch_stats3(v, nx, ny, nz, R3, x, y, z, mean, var);
 }
 
 void oracle_box_moments(const float *v, int nx, int ny, int nz, int R, double *mean, double *var) {
@@ -425,4 +433,392 @@ void oracle_register_mode(const float *ct, const float *cbct, int nx, int ny, in
 void oracle_register(const float *ct, const float *cbct, int nx, int ny, int nz, int R, double sigma, int levels,
                      int iters, double eps_var, double eps_den, float *out_disp, float *out_corr, double *trace) {
     oracle_register_mode(ct, cbct, nx, ny, nz, R, sigma, levels, iters, eps_var, eps_den, 0, out_disp, out_corr, trace);
+}
+
+/* ========================================================================
+ * Extensions for SURVEY.md section 8(f): NEXT-4 (per-axis patch radius and
+ * pyramid factor), NEXT-1 (reliability mask + interpolation of a, b), the
+ * Fig.-9 diagnostics, and the summed-area moments used between the first and
+ * last iteration of a level in config 4's whole-schedule check (SURVEY.md
+ * section 8(c) "Oracle cost").  Same conventions as above.
+ * ====================================================================== */
+
+/* NEXT-4: non-cubic patches (PAPER.md:386 lists 3x3x3 ... 25x25x7): radius R[c] along axis c. */
+void oracle_box_moments3(const float *v, int nx, int ny, int nz, const int R[3], double *mean, double *var) {
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) patch_stats3(v, nx, ny, nz, R, x, y, z, &mean[IDX(x, y, z)], &var[IDX(x, y, z)]);
+}
+
+/* The same truncated-patch moments by fp64 summed-area tables: an independently written O(1)-per-voxel routine,
+ * pinned against the naive loops above (tests/test_oracle_pins.py::test_sat_moments_match_naive).  The data are
+ * centred on the volume mean first (the variance is shift-invariant, the mean gets the shift back), the tables are
+ * three separable cumulative sums, the box sum is the 8-corner inclusion-exclusion, var = E(d^2) - E(d)^2
+ * (A.4) clamped at 0. */
+void oracle_box_moments_sat(const float *v, int nx, int ny, int nz, const int R[3], double *mean, double *var) {
+    const size_t N = (size_t)nx * ny * nz;
+    const int px = nx + 1, py = ny + 1, pz = nz + 1;
+    const size_t NP = (size_t)px * py * pz;
+#define PIDX(x, y, z) (((size_t)(z) * py + (y)) * px + (x))
+    double c = 0.0;
+    for (size_t i = 0; i < N; ++i) c += v[i];
+    c /= (double)N;
+    double *P1 = (double *)calloc(NP, sizeof(double)), *P2 = (double *)calloc(NP, sizeof(double));
+    /* P[z+1][y+1][x+1] = sum over the box [0..x] x [0..y] x [0..z]; index 0 planes stay zero */
+#pragma omp parallel for schedule(static)
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y) {
+            double r1 = 0.0, r2 = 0.0;                                  /* cumulative sum along x */
+            for (int x = 0; x < nx; ++x) {
+                double d = (double)v[IDX(x, y, z)] - c;
+                r1 += d; r2 += d * d;
+                P1[PIDX(x + 1, y + 1, z + 1)] = r1; P2[PIDX(x + 1, y + 1, z + 1)] = r2;
+            }
+        }
+#pragma omp parallel for schedule(static)
+    for (int z = 1; z <= nz; ++z)                                       /* ... along y */
+        for (int y = 2; y <= ny; ++y)
+            for (int x = 1; x <= nx; ++x) {
+                P1[PIDX(x, y, z)] += P1[PIDX(x, y - 1, z)]; P2[PIDX(x, y, z)] += P2[PIDX(x, y - 1, z)];
+            }
+#pragma omp parallel for schedule(static)
+    for (int y = 1; y <= ny; ++y)                                       /* ... along z */
+        for (int z = 2; z <= nz; ++z)
+            for (int x = 1; x <= nx; ++x) {
+                P1[PIDX(x, y, z)] += P1[PIDX(x, y, z - 1)]; P2[PIDX(x, y, z)] += P2[PIDX(x, y, z - 1)];
+            }
+#pragma omp parallel for schedule(static)
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) {
+                int x0 = clampi(x - R[0], 0, nx - 1), x1 = clampi(x + R[0], 0, nx - 1) + 1;
+                int y0 = clampi(y - R[1], 0, ny - 1), y1 = clampi(y + R[1], 0, ny - 1) + 1;
+                int z0 = clampi(z - R[2], 0, nz - 1), z1 = clampi(z + R[2], 0, nz - 1) + 1;
+                double n = (double)(x1 - x0) * (y1 - y0) * (z1 - z0);
+#define BOX(P) (P[PIDX(x1, y1, z1)] - P[PIDX(x0, y1, z1)] - P[PIDX(x1, y0, z1)] - P[PIDX(x1, y1, z0)] \
+              + P[PIDX(x0, y0, z1)] + P[PIDX(x0, y1, z0)] + P[PIDX(x1, y0, z0)] - P[PIDX(x0, y0, z0)])
+                double e1 = BOX(P1) / n, e2 = BOX(P2) / n;
+#undef BOX
+                double q = e2 - e1 * e1;
+                mean[IDX(x, y, z)] = e1 + c;
+                var[IDX(x, y, z)] = q > 0.0 ? q : 0.0;
+            }
+#undef PIDX
+    free(P1); free(P2);
+}
+
+/* NEXT-4: pyramid with a per-axis factor f[c] in {1, 2} (the paper's own preprocessing halves only the transverse
+ * plane).  Down: block mean over f[0] x f[1] x f[2] voxels.  Up: along an axis with factor 2 the
+ * cell-centre-aligned coordinate i/2 - 1/4 and component value x2 (reading A9); along an axis with factor 1 the
+ * coordinate i and component value x1 -- component c is in voxel units of axis c. */
+void oracle_downsample3(const float *v, int nx, int ny, int nz, const int f[3], float *out) {
+    int mx = nx / f[0], my = ny / f[1], mz = nz / f[2];
+#pragma omp parallel for schedule(static)
+    for (int z = 0; z < mz; ++z)
+        for (int y = 0; y < my; ++y)
+            for (int x = 0; x < mx; ++x) {
+                double s = 0.0;
+                for (int c = 0; c < f[2]; ++c)
+                    for (int b = 0; b < f[1]; ++b)
+                        for (int a = 0; a < f[0]; ++a) s += v[IDX(f[0] * x + a, f[1] * y + b, f[2] * z + c)];
+                out[((size_t)z * my + y) * mx + x] = (float)(s / (double)(f[0] * f[1] * f[2]));
+            }
+}
+
+void oracle_upsample_field3(const float *dc, int cx, int cy, int cz, const int f[3], float *out) {
+    int nx = f[0] * cx, ny = f[1] * cy, nz = f[2] * cz;
+    size_t Nc = (size_t)cx * cy * cz, N = (size_t)nx * ny * nz;
+    for (int comp = 0; comp < 3; ++comp) {
+        const float *src = dc + comp * Nc;
+        float *dst = out + comp * N;
+        double scale = (double)f[comp];
+#pragma omp parallel for schedule(static)
+        for (int z = 0; z < nz; ++z)
+            for (int y = 0; y < ny; ++y)
+                for (int x = 0; x < nx; ++x) {
+                    double px = f[0] == 2 ? x / 2.0 - 0.25 : (double)x;
+                    double py = f[1] == 2 ? y / 2.0 - 0.25 : (double)y;
+                    double pz = f[2] == 2 ? z / 2.0 - 0.25 : (double)z;
+                    dst[IDX(x, y, z)] = (float)(scale * trilinear(src, cx, cy, cz, px, py, pz));
+                }
+    }
+}
+
+/* ------------------------------------------------------------------------
+ * NEXT-1: reliability mask and interpolation / extrapolation of a, b
+ * (Eqs. (5)-(10); parameters PAPER.md:161, :165).
+ * ---------------------------------------------------------------------- */
+
+/* Eqs. (5), (6) from given patch moments: a = STD(M)/STD(S) (0 where var_s <= eps_var, reading A5),
+ * b = E(M) - a E(S). */
+void oracle_ab_from_moments(const double *mu_s, const double *var_s, const double *mu_m, const double *var_m, size_t N,
+                            double eps_var, double *a, double *b) {
+#pragma omp parallel for schedule(static)
+    for (long long i = 0; i < (long long)N; ++i) {
+        double ai = var_s[i] > eps_var ? sqrt(var_m[i] / var_s[i]) : 0.0;
+        a[i] = ai; b[i] = mu_m[i] - ai * mu_s[i];
+    }
+}
+
+/* Eq. (7) (printed as a broken `cases`): xi = 1 where |I_m^(k)(x) - I_s(x)| > HU_0 or
+ * a(x) < a_min or a(x) > a_max, 0 elsewhere.  Comparisons in fp64 (the difference of two fp32 values is exact). */
+void oracle_mask(const float *m, const float *cbct, const double *a, size_t N, double hu0, double a_min, double a_max,
+                 unsigned char *xi) {
+#pragma omp parallel for schedule(static)
+    for (long long i = 0; i < (long long)N; ++i) {
+        double d = fabs((double)m[i] - (double)cbct[i]);
+        xi[i] = (d > hu0 || a[i] < a_min || a[i] > a_max) ? 1 : 0;
+    }
+}
+
+/* Eqs. (8)-(10): "Initially, we set a(x)=0 and b(x)=0 for xi(x)=1"; then every voxel with xi = 1
+ * takes the weighted average of the a, b of the AVAILABLE voxels (xi = 0, or filled by an earlier pass) inside the
+ * cube T of radius RT centred at it (truncated to the volume), w_i = exp(-(I_s(i) - I_s(x))^2 / h^2); the pass is
+ * repeated "since for some voxels the values of xi may be 1 for all voxels in their neighbor T".  Values at
+ * xi = 0 voxels are never changed.  Readings (A18): a pass reads only what was available when it
+ * started (Jacobi); the weights are normalised by the largest one, w_i = exp(-((D_i)^2 - min_j (D_j)^2) / h^2), which
+ * is the same quotient as Eqs. (8)-(9) and cannot underflow to 0/0; passes stop when nothing is left, when a pass
+ * fills nothing, or after max_passes; what is still unfilled keeps a = b = 0.
+ * xi (in/out): 1 = masked and unfilled; on return 1 only where no value could be found.  Returns the passes run. */
+int oracle_fill_ab(const float *cbct, int nx, int ny, int nz, unsigned char *xi, double *a, double *b, int RT, double h,
+                   int max_passes) {
+    const size_t N = (size_t)nx * ny * nz;
+    unsigned char *nxt = (unsigned char *)malloc(N);
+    double *na = (double *)malloc(sizeof(double) * N), *nb = (double *)malloc(sizeof(double) * N);
+    for (size_t i = 0; i < N; ++i)
+        if (xi[i]) { a[i] = 0.0; b[i] = 0.0; }
+    int pass = 0;
+    for (; pass < max_passes; ++pass) {
+        long long left = 0, filled = 0;
+        for (size_t i = 0; i < N; ++i) left += xi[i];
+        if (left == 0) break;
+        memcpy(nxt, xi, N);
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : filled)
+        for (int z = 0; z < nz; ++z)
+            for (int y = 0; y < ny; ++y)
+                for (int x = 0; x < nx; ++x) {
+                    size_t i0 = IDX(x, y, z);
+                    if (!xi[i0]) continue;
+                    double s0 = cbct[i0], dmin = INFINITY;
+                    int x0 = clampi(x - RT, 0, nx - 1), x1 = clampi(x + RT, 0, nx - 1);
+                    int y0 = clampi(y - RT, 0, ny - 1), y1 = clampi(y + RT, 0, ny - 1);
+                    int z0 = clampi(z - RT, 0, nz - 1), z1 = clampi(z + RT, 0, nz - 1);
+                    for (int c = z0; c <= z1; ++c)
+                        for (int bb = y0; bb <= y1; ++bb)
+                            for (int aa = x0; aa <= x1; ++aa) {
+                                size_t i = IDX(aa, bb, c);
+                                if (xi[i]) continue;
+                                double d = (double)cbct[i] - s0;
+                                if (d * d < dmin) dmin = d * d;
+                            }
+                    if (dmin == INFINITY) continue;               /* every voxel of T is still masked */
+                    double sw = 0.0, sa = 0.0, sb = 0.0;
+                    for (int c = z0; c <= z1; ++c)
+                        for (int bb = y0; bb <= y1; ++bb)
+                            for (int aa = x0; aa <= x1; ++aa) {
+                                size_t i = IDX(aa, bb, c);
+                                if (xi[i]) continue;
+                                double d = (double)cbct[i] - s0;
+                                double w = exp(-(d * d - dmin) / (h * h));  /* Eq. (10) */
+                                sw += w; sa += w * a[i]; sb += w * b[i];
+                            }
+                    na[i0] = sa / sw; nb[i0] = sb / sw;           /* Eqs. (8), (9) */
+                    nxt[i0] = 0;
+                    ++filled;
+                }
+        for (size_t i = 0; i < N; ++i)
+            if (xi[i] && !nxt[i]) { a[i] = na[i]; b[i] = nb[i]; }
+        memcpy(xi, nxt, N);
+        if (filled == 0) { ++pass; break; }
+    }
+    free(nxt); free(na); free(nb);
+    return pass;
+}
+
+/* I'_s = a I_s + b on the original static image. */
+void oracle_apply_ab(const float *cbct, const double *a, const double *b, size_t N, float *out) {
+#pragma omp parallel for schedule(static)
+    for (long long i = 0; i < (long long)N; ++i) out[i] = (float)(a[i] * (double)cbct[i] + b[i]);
+}
+
+/* Delta HU = mean(CT) - mean(CBCT), the constant that shifts the CBCT to the CT's mean intensity. */
+double oracle_delta_hu(const float *ct, const float *cbct, size_t N) {
+    double s1 = 0.0, s2 = 0.0;
+    for (size_t i = 0; i < N; ++i) { s1 += ct[i]; s2 += cbct[i]; }
+    return (s1 - s2) / (double)N;
+}
+
+static int cmp_double(const void *p, const void *q) {
+    double a = *(const double *)p, b = *(const double *)q;
+    return a < b ? -1 : (a > b ? 1 : 0);
+}
+
+/* "A is calculated before starting DIR and the median value a_m of A is used".  Reading A17: the
+ * median runs over the voxels where Eq. (5) is a ratio of two positive deviations (var_s > eps_var and
+ * var_m > eps_var) and is the lower median (order statistic floor((n-1)/2)); 1 if there is no such voxel. */
+double oracle_median_a(const double *a, const double *var_s, const double *var_m, size_t N, double eps_var) {
+    double *t = (double *)malloc(sizeof(double) * (N ? N : 1));
+    size_t n = 0;
+    for (size_t i = 0; i < N; ++i)
+        if (var_s[i] > eps_var && var_m[i] > eps_var) t[n++] = a[i];
+    double med = 1.0;
+    if (n) { qsort(t, n, sizeof(double), cmp_double); med = t[(n - 1) / 2]; }
+    free(t);
+    return med;
+}
+
+/* ------------------------------------------------------------------------
+ * The general driver: Algorithm A1 with every option.
+ * ---------------------------------------------------------------------- */
+typedef struct {
+    int R[3];             /* patch radius per axis */
+    int fac[3];           /* pyramid factor per axis, 1 or 2 */
+    double sigma;         /* Gaussian sigma in voxels */
+    int levels, iters;
+    double eps_var, eps_den;
+    int double_force;     /* both terms of Eq. (1) */
+    double stop_eps;      /* < 0: fixed iteration count */
+    int moments_policy;   /* 0: naive patch loops always; 1: summed-area tables except in the first and last iteration of a level */
+    /* NEXT-1 */
+    int mask;             /* 1: A1 "globally adjust", step 2 and Eq. (7) are on */
+    double hu0;           /* < 0: HU_0 = 2 |Delta HU| */
+    double a_min, a_max;  /* a_min < 0: 0.5 a_m and 1.5 a_m with a_m = median(A) before the DIR */
+    int fill_radius;      /* radius of T (PAPER.md:131; its size is lost from the text, :165) */
+    double h;             /* Eq. (10); never given */
+    int max_fill_passes;
+} oracle_params;
+
+typedef struct {
+    double delta_hu, hu0, a_m, a_min, a_max;   /* what the mask used */
+} oracle_info;
+
+static void level_dims(const oracle_params *p, int nx, int ny, int nz, int l, int *lx, int *ly, int *lz) {
+    *lx = nx; *ly = ny; *lz = nz;
+    for (int i = 0; i < l; ++i) { *lx /= p->fac[0]; *ly /= p->fac[1]; *lz /= p->fac[2]; }
+}
+
+static void moments_by_policy(const oracle_params *p, int k, int n_it, const float *v, int lx, int ly, int lz, double *mean,
+                              double *var) {
+    if (p->moments_policy == 1 && k > 0 && k < n_it - 1) oracle_box_moments_sat(v, lx, ly, lz, p->R, mean, var);
+    else oracle_box_moments3(v, lx, ly, lz, p->R, mean, var);
+}
+
+/* A1 steps 1 (second half) to 3 from given patch moments: a, b by Eqs. (5)-(6); with the mask on, Eq. (7), the
+ * interpolation of Eqs. (8)-(10) and I'_s = a I_s + b; without it the same correction written as
+ * a (I_s - mu_s) + mu_m (the hot path's form). */
+static void correct_step(const oracle_params *p, const oracle_info *inf, const float *cbct, const float *m, int lx, int ly,
+                         int lz, const double *mus, const double *vs, const double *mum, const double *vm, double *a,
+                         double *b, unsigned char *xi, float *sp) {
+    const size_t N = (size_t)lx * ly * lz;
+    oracle_ab_from_moments(mus, vs, mum, vm, N, p->eps_var, a, b);
+    if (p->mask) {
+        oracle_mask(m, cbct, a, N, inf->hu0, inf->a_min, inf->a_max, xi);                      /* Eq. (7) */
+        oracle_fill_ab(cbct, lx, ly, lz, xi, a, b, p->fill_radius, p->h, p->max_fill_passes);   /* A1 step 2 */
+        oracle_apply_ab(cbct, a, b, N, sp);                                                    /* A1 step 3 */
+    } else {
+        oracle_correct_from_moments(cbct, mus, vs, mum, vm, N, p->eps_var, sp);                 /* A1 step 3 */
+    }
+}
+
+/* Outputs (each may be NULL except out_disp): out_corr [N0]; iters_run [levels]; ltrace, mean_a, mean_b
+ * [levels*iters], level-major from the coarsest level (l(k), and Fig. 9 (e),(f): the averages of a and b over all
+ * voxels in every iteration); info. */
+void oracle_register_ex(const float *ct, const float *cbct_in, int nx, int ny, int nz, const oracle_params *p,
+                        float *out_disp, float *out_corr, int *iters_run, double *ltrace, double *mean_a, double *mean_b,
+                        oracle_info *info) {
+    const int levels = p->levels;
+    const size_t N0 = (size_t)nx * ny * nz;
+    oracle_info inf = {0.0, 0.0, 1.0, 0.0, 0.0};
+    float *cbct0 = (float *)malloc(sizeof(float) * N0);
+    memcpy(cbct0, cbct_in, sizeof(float) * N0);
+    if (p->mask) {
+        /* A1 "Globally adjust the intensity of CBCT" */
+        inf.delta_hu = oracle_delta_hu(ct, cbct_in, N0);
+        for (size_t i = 0; i < N0; ++i) cbct0[i] = (float)((double)cbct_in[i] + inf.delta_hu);
+        inf.hu0 = p->hu0 >= 0.0 ? p->hu0 : 2.0 * fabs(inf.delta_hu);
+        if (p->a_min >= 0.0) { inf.a_min = p->a_min; inf.a_max = p->a_max; }
+        else {
+            /* A before the DIR (r = 0, full resolution), a_m = median(A) */
+            double *mus = (double *)malloc(sizeof(double) * N0), *vs = (double *)malloc(sizeof(double) * N0);
+            double *mum = (double *)malloc(sizeof(double) * N0), *vm = (double *)malloc(sizeof(double) * N0);
+            double *a = (double *)malloc(sizeof(double) * N0), *b = (double *)malloc(sizeof(double) * N0);
+            oracle_box_moments3(cbct0, nx, ny, nz, p->R, mus, vs);
+            oracle_box_moments3(ct, nx, ny, nz, p->R, mum, vm);
+            oracle_ab_from_moments(mus, vs, mum, vm, N0, p->eps_var, a, b);
+            inf.a_m = oracle_median_a(a, vs, vm, N0, p->eps_var);
+            inf.a_min = 0.5 * inf.a_m; inf.a_max = 1.5 * inf.a_m;
+            free(mus); free(vs); free(mum); free(vm); free(a); free(b);
+        }
+    }
+    const float **pct = (const float **)malloc(sizeof(float *) * levels);
+    const float **pcb = (const float **)malloc(sizeof(float *) * levels);
+    pct[0] = ct; pcb[0] = cbct0;
+    for (int l = 1; l < levels; ++l) {
+        int fx, fy, fz;
+        level_dims(p, nx, ny, nz, l - 1, &fx, &fy, &fz);
+        size_t Nl = (size_t)(fx / p->fac[0]) * (fy / p->fac[1]) * (fz / p->fac[2]);
+        float *a = (float *)malloc(sizeof(float) * Nl), *b = (float *)malloc(sizeof(float) * Nl);
+        oracle_downsample3(pct[l - 1], fx, fy, fz, p->fac, a);
+        oracle_downsample3(pcb[l - 1], fx, fy, fz, p->fac, b);
+        pct[l] = a; pcb[l] = b;
+    }
+    float *r = NULL;
+    for (int l = levels - 1; l >= 0; --l) {
+        int lx, ly, lz;
+        level_dims(p, nx, ny, nz, l, &lx, &ly, &lz);
+        size_t N = (size_t)lx * ly * lz;
+        if (r == NULL) r = (float *)calloc(3 * N, sizeof(float));
+        else {
+            float *rf = (float *)malloc(sizeof(float) * 3 * N);
+            oracle_upsample_field3(r, lx / p->fac[0], ly / p->fac[1], lz / p->fac[2], p->fac, rf);
+            free(r); r = rf;
+        }
+        float *m = (float *)malloc(sizeof(float) * N), *sp = (float *)malloc(sizeof(float) * N);
+        double *mus = (double *)malloc(sizeof(double) * N), *vs = (double *)malloc(sizeof(double) * N);
+        double *mum = (double *)malloc(sizeof(double) * N), *vm = (double *)malloc(sizeof(double) * N);
+        double *a = (double *)malloc(sizeof(double) * N), *b = (double *)malloc(sizeof(double) * N);
+        unsigned char *xi = (unsigned char *)malloc(N);
+        oracle_box_moments3(pcb[l], lx, ly, lz, p->R, mus, vs);
+        const int n_it = p->iters;
+        int k_run = 0;
+        double *hist = (double *)malloc(sizeof(double) * (n_it > 0 ? n_it : 1));
+        for (int k = 0; k < n_it; ++k) {
+            oracle_warp(pct[l], r, lx, ly, lz, m);                                  /* I_m^(k) */
+            moments_by_policy(p, k, n_it, m, lx, ly, lz, mum, vm);                  /* A1 step 1 */
+            correct_step(p, &inf, pcb[l], m, lx, ly, lz, mus, vs, mum, vm, a, b, xi, sp);   /* A1 steps 1-3 */
+            if (mean_a || mean_b) {
+                double sa = 0.0, sb = 0.0;
+                for (size_t i = 0; i < N; ++i) { sa += a[i]; sb += b[i]; }
+                if (mean_a) mean_a[(size_t)(levels - 1 - l) * n_it + k] = sa / (double)N;
+                if (mean_b) mean_b[(size_t)(levels - 1 - l) * n_it + k] = sb / (double)N;
+            }
+            int stop = 0;
+            if (p->stop_eps >= 0.0 || ltrace) {
+                double sdr, sr;
+                oracle_force_norms(m, sp, r, lx, ly, lz, p->eps_den, p->double_force, &sdr, &sr);
+                hist[k] = sr > 0.0 ? sdr / sr : INFINITY;
+                if (ltrace) ltrace[(size_t)(levels - 1 - l) * n_it + k] = hist[k];
+                if (p->stop_eps >= 0.0 && k >= 10 && hist[k - 10] - hist[k] <= p->stop_eps) stop = 1;
+            }
+            if (p->double_force) oracle_force_update_double(m, sp, lx, ly, lz, p->eps_den, r);
+            else oracle_force_update(m, sp, lx, ly, lz, p->eps_den, r);             /* A1 steps 4-5 */
+            oracle_smooth_field(r, lx, ly, lz, p->sigma);                           /* A1 step 6 */
+            k_run = k + 1;
+            if (stop) break;
+        }
+        if (l == 0 && out_corr) {                                                   /* reading A12 */
+            oracle_warp(pct[0], r, lx, ly, lz, m);
+            oracle_box_moments3(m, lx, ly, lz, p->R, mum, vm);
+            correct_step(p, &inf, pcb[0], m, lx, ly, lz, mus, vs, mum, vm, a, b, xi, out_corr);
+        }
+        free(hist);
+        if (iters_run) iters_run[l] = k_run;
+        if (l == 0) memcpy(out_disp, r, sizeof(float) * 3 * N);
+        free(m); free(sp); free(mus); free(vs); free(mum); free(vm); free(a); free(b); free(xi);
+    }
+    free(r);
+    for (int l = 1; l < levels; ++l) { free((void *)pct[l]); free((void *)pcb[l]); }
+    free(pct); free(pcb); free(cbct0);
+    if (info) *info = inf;
 }
