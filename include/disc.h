@@ -42,7 +42,7 @@ typedef enum {
 } disc_status;
 
 /* Limits of this build. */
-#define DISC_MAX_PATCH_RADIUS 10
+#define DISC_MAX_PATCH_RADIUS 12
 #define DISC_MAX_GAUSS_RADIUS 12 /* ceil(3*sigma) <= 12, i.e. sigma <= 4 */
 #define DISC_MAX_LEVELS 8
 

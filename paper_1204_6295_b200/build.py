@@ -18,17 +18,10 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libdisc.so")
 
 # no --use_fast_math: IEEE division and sqrt are kept
-NVCC_FLAGS = os.environ.get("DISC_EXTRA_FLAGS", "").split() + ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 R_RANGES = [(0, 3), (4, 5), (6, 7), (8, 10)]
 K_RANGES = [(1, 3), (4, 6), (7, 9), (10, 12)]
-# development shortcut: DISC_DEV_RK="R,K" instantiates only that patch radius and Gaussian radius (seconds instead of
-# minutes); every other R / K then reports DISC_ERR_UNSUPPORTED.  Never set for a build that is tested or shipped.
-if os.environ.get("DISC_DEV_RK"):
-    _r, _k = (int(v) for v in os.environ["DISC_DEV_RK"].split(","))
-    R_RANGES = [(_r, _r)] + [(99, 98)] * 3
-    K_RANGES = [(_k, _k)] + [(99, 98)] * 3
-
 
 def _units():
     units = [("disc_api", "disc_api.cu", [])]

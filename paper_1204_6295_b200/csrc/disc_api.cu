@@ -32,10 +32,6 @@ thread_local char g_create_error[256] = "";
 
 }  // namespace
 
-namespace disc {
-thread_local IterCtl g_iter_ctl = {nullptr, 0};
-}
-
 struct disc_ctx {
     int dims[3];
     float spacing[3];
@@ -47,7 +43,7 @@ struct disc_ctx {
     float stop_eps;   // < 0: stopping criterion off (default)
     StopCtl* d_stop;  // device-side state of the criterion
     int runs_host[DISC_MAX_LEVELS];   // iterations per level when the criterion is off
-    int n_sm;
+    DevInfo di;       // device the context was created on, and its SM count
     GaussTaps taps;
     Level lv[DISC_MAX_LEVELS];
     float* h2d_ct;    // device staging for disc_register_host
@@ -86,83 +82,41 @@ disc_status check_launch(disc_ctx* c, const char* what) {
         if (!(cond)) return fail((c), DISC_ERR_INVALID_ARG, "%s", (msg));   \
     } while (0)
 
-// optional launch-shape overrides for tuning sweeps (unset in normal use)
-int tune(const char* name, int dflt) {
-    const char* v = std::getenv(name);
-    return v && *v ? std::atoi(v) : dflt;
-}
-
 bool level_ok(const disc_ctx* c, int level) { return level >= 0 && level < c->levels; }
 
-int pick_chunk(int n, int min_chunk, long long ctas_per_chunk, long long target_ctas) {
-    // split an axis of length n into chunks so that the grid reaches ~target_ctas CTAs,
-    // but never below min_chunk (each chunk re-reads a halo)
-    long long want = target_ctas / ctas_per_chunk;  // round down: prefer one full wave over 1.x waves
-    if (want < 1) want = 1;
-    int chunk = (int)((n + want - 1) / want);
-    if (chunk < min_chunk) chunk = min_chunk;
-    if (chunk > n) chunk = n;
-    return chunk;
-}
+const IterCtl kNoCtl = {nullptr, 0};
 
-// ------------------------------------------------------------------ kernels instantiated in moments_tu.cu / field_tu.cu
-// Tile height and z chunk of the moments kernel: minimise (waves) x (slices marched per CTA, with the 2R halo)
-// x (rows per slice, with the x pass's 2R halo rows).  The 32x32 tile runs one CTA per SM, the 32x16 tile two.
-void pick_moments_shape(const disc_ctx* c, const Level& L, int* ty_out, int* zchunk_out) {
-    const int R = c->R;
-    double best = 1e300;
-    int best_ty = 16, best_zc = L.nz;
-    for (int ty = 16; ty <= 32; ty += 16) {
-        if (ty == 32 && R > kMomMaxRTile32) continue;
-        const long long tiles = (long long)((L.nx + 31) / 32) * ((L.ny + ty - 1) / ty);
-        const long long slots = (long long)c->n_sm * (ty == 16 ? 2 : 1);
-        for (int nchunk = 1; nchunk <= L.nz; ++nchunk) {
-            const int zc = (L.nz + nchunk - 1) / nchunk;
-            const long long ctas = tiles * ((L.nz + zc - 1) / zc);
-            const long long waves = (ctas + slots - 1) / slots;
-            const double cost = (double)waves * (zc + 2 * R + 6) * (ty + R + 4) * (ty == 16 ? 1.8 : 1.0);
-            if (cost < best) { best = cost; best_ty = ty; best_zc = zc; }
-            if (zc == 1) break;
-        }
-    }
-    *ty_out = tune("DISC_TUNE_MOM_TY", best_ty);
-    *zchunk_out = tune("DISC_TUNE_MOM_ZCHUNK", best_zc);
+// every entry point runs on the device the context was created on (scratch, attributes and grid sizes belong to it)
+disc_status check_device(disc_ctx* c) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return fail(c, DISC_ERR_CUDA, "cudaGetDevice failed");
+    if (dev != c->di.dev)
+        return fail(c, DISC_ERR_INVALID_ARG, "context belongs to CUDA device %d, current device is %d", c->di.dev, dev);
+    return DISC_OK;
 }
 
 template <int MODE>
 disc_status launch_moments(disc_ctx* c, const Level& L, const float* vol, const float* aux, float* out0,
-                           float* out1, cudaStream_t st) {
-    int ty, zchunk;
-    pick_moments_shape(c, L, &ty, &zchunk);
-    if (!launch_moments_any(c->R, MODE, ty, vol, aux, out0, out1, L.nx, L.ny, L.nz, zchunk, DISC_EPS_VAR, st))
-        return fail(c, DISC_ERR_UNSUPPORTED, "patch_radius %d > %d", c->R, DISC_MAX_PATCH_RADIUS);
+                           float* out1, IterCtl ctl, cudaStream_t st) {
+    if (!launch_moments_any(c->di, c->R, c->R, MODE, vol, aux, out0, out1, L.nx, L.ny, L.nz, DISC_EPS_VAR, ctl, st))
+        return fail(c, DISC_ERR_UNSUPPORTED, "no moments kernel for patch radius %d on %dx%dx%d", c->R, L.nx, L.ny, L.nz);
     return check_launch(c, "k_moments");
 }
 
 // force: 0 = plain smoothing, otherwise the context's force mode
 disc_status launch_force_gxy(disc_ctx* c, bool force, const Level& L, const float* m, const float* s, const float* rin,
-                             float* rout, cudaStream_t st) {
+                             float* rout, IterCtl ctl, cudaStream_t st) {
     const int FORCE = force ? c->force_mode : 0;
-    const int txb = L.nx > 64 ? 128 : (L.nx > 32 ? 64 : 32);
-    const int xt = (L.nx + txb - 1) / txb;
-    const int K = c->K;
-    const int yseg = tune("DISC_TUNE_FG_YSEG", pick_chunk(L.ny, 8 * K > 32 ? 8 * K : 32, (long long)xt * L.nz, 4 * 148));
-    if (!launch_force_gxy_any(K, FORCE, txb, m, s, rin, rout, L.nx, L.ny, L.nz, yseg, DISC_EPS_DEN, c->taps, st))
-        return fail(c, DISC_ERR_UNSUPPORTED, "Gaussian radius %d unsupported", K);
+    if (!launch_force_gxy_any(c->di, c->K, FORCE, m, s, rin, rout, L.nx, L.ny, L.nz, DISC_EPS_DEN, c->taps, ctl, st))
+        return fail(c, DISC_ERR_UNSUPPORTED, "Gaussian radius %d unsupported", c->K);
     return check_launch(c, "k_force_gxy");
 }
 
 template <bool WARP>
 disc_status launch_gz_warp(disc_ctx* c, const Level& L, const float* rin, float* rout, const float* moving,
-                           float* mout, cudaStream_t st) {
-    // a thread owns two adjacent columns and `lz` output slices (field_v3.cuh); measured on B200: with two columns
-    // per thread 4 slices beat 8 at every level (more threads in flight; the 2K halo re-reads come from L2)
-    const int K = c->K;
-    const int lz = tune("DISC_TUNE_GZ_LZ", 4);
-    const int cols = tune("DISC_TUNE_GZ_COLS", 2);   // columns per thread: 2 = packed (needs nx even), 1 = scalar
-    const int zchunk = lz + 100 * cols;
-    if (!launch_gz_warp_any(K, WARP, rin, rout, moving, mout, L.nx, L.ny, L.nz, zchunk, c->taps, st))
-        return fail(c, DISC_ERR_UNSUPPORTED, "Gaussian radius %d unsupported", K);
+                           float* mout, IterCtl ctl, cudaStream_t st) {
+    if (!launch_gz_warp_any(c->di, c->K, WARP, rin, rout, moving, mout, L.nx, L.ny, L.nz, c->taps, ctl, st))
+        return fail(c, DISC_ERR_UNSUPPORTED, "Gaussian radius %d unsupported", c->K);
     return check_launch(c, "k_gz_warp");
 }
 
@@ -197,22 +151,21 @@ disc_status iterate_level(disc_ctx* c, Level& L, const float* ct, float* disp, i
     for (int k = 0; k < n_iters && rc == DISC_OK; ++k) {
         // with the criterion on, every kernel of iteration k falls through once an earlier iteration has tripped it;
         // the field and L.m then stay those of the last iteration run (its z pass always refreshes L.m: k + 1 < n_iters)
-        g_iter_ctl = stop ? IterCtl{&c->d_stop->stop_iter, k} : IterCtl{nullptr, 0};
-        rc = launch_moments<kModeCorrect>(c, L, L.m, L.zhat, L.sp, nullptr, st);              // A1 steps 1,3
+        const IterCtl ctl = stop ? IterCtl{&c->d_stop->stop_iter, k} : kNoCtl;
+        rc = launch_moments<kModeCorrect>(c, L, L.m, L.zhat, L.sp, nullptr, ctl, st);         // A1 steps 1,3
         if (rc == DISC_OK && stop) {                                                           // PAPER.md:167, l^(k)
             launch_force_norms(c->force_mode, L.m, L.sp, disp, L.nx, L.ny, L.nz, DISC_EPS_DEN, c->d_stop, k, c->stop_eps,
-                               c->n_sm, st);
+                               c->di.n_sm, st);
             rc = check_launch(c, "k_force_norms");
         }
-        if (rc == DISC_OK) rc = launch_force_gxy(c, true, L, L.m, L.sp, disp, L.scratch, st);  // A1 steps 4,5,6(x,y)
+        if (rc == DISC_OK) rc = launch_force_gxy(c, true, L, L.m, L.sp, disp, L.scratch, ctl, st);  // A1 steps 4,5,6(x,y)
         if (rc == DISC_OK) {
             if (k + 1 < n_iters || final_warp)
-                rc = launch_gz_warp<true>(c, L, L.scratch, disp, ct, L.m, st);                 // A1 step 6(z) + next I_m^(k)
+                rc = launch_gz_warp<true>(c, L, L.scratch, disp, ct, L.m, ctl, st);            // A1 step 6(z) + next I_m^(k)
             else
-                rc = launch_gz_warp<false>(c, L, L.scratch, disp, nullptr, nullptr, st);
+                rc = launch_gz_warp<false>(c, L, L.scratch, disp, nullptr, nullptr, ctl, st);
         }
     }
-    g_iter_ctl = IterCtl{nullptr, 0};
     if (rc == DISC_OK && stop) { launch_stop_record(c->d_stop, level, n_iters, st); rc = check_launch(c, "k_stop_record"); }
     return rc;
 }
@@ -261,13 +214,15 @@ disc_status disc_create(disc_ctx** out, const int dims[3], const float spacing[3
     e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
     if (e != cudaSuccess) return fail(nullptr, DISC_ERR_CUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e));
     if (major != 10) return fail(nullptr, DISC_ERR_UNSUPPORTED, "device compute capability %d.x, this library is sm_100a only", major);
+    if (dev < 0 || dev >= kMaxDevices) return fail(nullptr, DISC_ERR_UNSUPPORTED, "device ordinal %d >= %d", dev, kMaxDevices);
 
     disc_ctx* c = new (std::nothrow) disc_ctx();
     if (!c) return fail(nullptr, DISC_ERR_ALLOC, "out of host memory");
     std::memset(c, 0, sizeof(*c));
     for (int i = 0; i < 3; ++i) { c->dims[i] = dims[i]; c->spacing[i] = spacing[i]; }
-    c->n_sm = 148;
-    cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
+    c->di.dev = dev;
+    c->di.n_sm = 148;
+    cudaDeviceGetAttribute(&c->di.n_sm, cudaDevAttrMultiProcessorCount, dev);
     c->R = patch_radius; c->sigma = sigma_smooth; c->levels = levels; c->iters = iters; c->K = K;
     c->force_mode = DISC_FORCE_THIRION;
     c->stop_eps = -1.f;
@@ -343,6 +298,7 @@ disc_status disc_iterations_run(disc_ctx* c, int* out_host) {
 
 disc_status disc_warp(disc_ctx* c, int level, const float* moving, const float* disp, float* out, void* stream) {
     if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
     DISC_NEED(c, level_ok(c, level), "level out of range");
     DISC_NEED(c, moving && disp && out, "NULL pointer");
     return launch_warp(c, c->lv[level], moving, disp, out, (cudaStream_t)stream);
@@ -351,34 +307,37 @@ disc_status disc_warp(disc_ctx* c, int level, const float* moving, const float* 
 disc_status disc_correct_intensity(disc_ctx* c, int level, const float* cbct, const float* ct_warped,
                                    float* out_corrected, void* stream) {
     if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
     DISC_NEED(c, level_ok(c, level), "level out of range");
     DISC_NEED(c, cbct && ct_warped && out_corrected, "NULL pointer");
     Level& L = c->lv[level];
     cudaStream_t st = (cudaStream_t)stream;
-    DISC_TRY(launch_moments<kModeZscore>(c, L, cbct, nullptr, L.zhat, nullptr, st));
-    return launch_moments<kModeCorrect>(c, L, ct_warped, L.zhat, out_corrected, nullptr, st);
+    DISC_TRY(launch_moments<kModeZscore>(c, L, cbct, nullptr, L.zhat, nullptr, kNoCtl, st));
+    return launch_moments<kModeCorrect>(c, L, ct_warped, L.zhat, out_corrected, nullptr, kNoCtl, st);
 }
 
 disc_status disc_demons_step(disc_ctx* c, int level, const float* m_warped, const float* s_corrected,
                              float* disp_inout, void* stream) {
     if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
     DISC_NEED(c, level_ok(c, level), "level out of range");
     DISC_NEED(c, m_warped && s_corrected && disp_inout, "NULL pointer");
     Level& L = c->lv[level];
     cudaStream_t st = (cudaStream_t)stream;
-    DISC_TRY(launch_force_gxy(c, true, L, m_warped, s_corrected, disp_inout, L.scratch, st));
-    return launch_gz_warp<false>(c, L, L.scratch, disp_inout, nullptr, nullptr, st);
+    DISC_TRY(launch_force_gxy(c, true, L, m_warped, s_corrected, disp_inout, L.scratch, kNoCtl, st));
+    return launch_gz_warp<false>(c, L, L.scratch, disp_inout, nullptr, nullptr, kNoCtl, st);
 }
 
 disc_status disc_iterate(disc_ctx* c, int level, const float* ct, const float* cbct, float* disp_inout,
                          int n_iters, void* stream) {
     if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
     DISC_NEED(c, level_ok(c, level), "level out of range");
     DISC_NEED(c, ct && cbct && disp_inout, "NULL pointer");
     DISC_NEED(c, n_iters >= 0, "n_iters < 0");
     Level& L = c->lv[level];
     cudaStream_t st = (cudaStream_t)stream;
-    DISC_TRY(launch_moments<kModeZscore>(c, L, cbct, nullptr, L.zhat, nullptr, st));
+    DISC_TRY(launch_moments<kModeZscore>(c, L, cbct, nullptr, L.zhat, nullptr, kNoCtl, st));
     DISC_TRY(launch_warp(c, L, ct, disp_inout, L.m, st));
     return iterate_level(c, L, ct, disp_inout, n_iters, true, st);
 }
@@ -386,6 +345,7 @@ disc_status disc_iterate(disc_ctx* c, int level, const float* ct, const float* c
 disc_status disc_profile_iteration(disc_ctx* c, int level, const float* ct, const float* cbct, float* disp_inout,
                                    int n_iters, float ms_per_kernel[3], void* stream) {
     if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
     DISC_NEED(c, level_ok(c, level), "level out of range");
     DISC_NEED(c, ct && cbct && disp_inout && ms_per_kernel, "NULL pointer");
     DISC_NEED(c, n_iters >= 1 && n_iters <= 4096, "n_iters must be in 1..4096");
@@ -395,15 +355,15 @@ disc_status disc_profile_iteration(disc_ctx* c, int level, const float* ct, cons
     cudaEvent_t* ev = new (std::nothrow) cudaEvent_t[ne];
     if (!ev) return fail(c, DISC_ERR_ALLOC, "out of host memory");
     for (int i = 0; i < ne; ++i) cudaEventCreate(&ev[i]);
-    disc_status rc = launch_moments<kModeZscore>(c, L, cbct, nullptr, L.zhat, nullptr, st);
+    disc_status rc = launch_moments<kModeZscore>(c, L, cbct, nullptr, L.zhat, nullptr, kNoCtl, st);
     if (rc == DISC_OK) rc = launch_warp(c, L, ct, disp_inout, L.m, st);
     for (int k = 0; k < n_iters && rc == DISC_OK; ++k) {
         cudaEventRecord(ev[4 * k + 0], st);
-        rc = launch_moments<kModeCorrect>(c, L, L.m, L.zhat, L.sp, nullptr, st);
+        rc = launch_moments<kModeCorrect>(c, L, L.m, L.zhat, L.sp, nullptr, kNoCtl, st);
         cudaEventRecord(ev[4 * k + 1], st);
-        if (rc == DISC_OK) rc = launch_force_gxy(c, true, L, L.m, L.sp, disp_inout, L.scratch, st);
+        if (rc == DISC_OK) rc = launch_force_gxy(c, true, L, L.m, L.sp, disp_inout, L.scratch, kNoCtl, st);
         cudaEventRecord(ev[4 * k + 2], st);
-        if (rc == DISC_OK) rc = launch_gz_warp<true>(c, L, L.scratch, disp_inout, ct, L.m, st);
+        if (rc == DISC_OK) rc = launch_gz_warp<true>(c, L, L.scratch, disp_inout, ct, L.m, kNoCtl, st);
         cudaEventRecord(ev[4 * k + 3], st);
     }
     cudaError_t e = cudaStreamSynchronize(st);
@@ -426,6 +386,7 @@ disc_status disc_profile_iteration(disc_ctx* c, int level, const float* ct, cons
 disc_status disc_register(disc_ctx* c, const float* ct, const float* cbct, float* out_disp,
                           float* out_corrected_cbct, void* stream) {
     if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
     DISC_NEED(c, ct && cbct && out_disp, "NULL pointer");
     cudaStream_t st = (cudaStream_t)stream;
     const int nl = c->levels;
@@ -447,12 +408,12 @@ disc_status disc_register(disc_ctx* c, const float* ct, const float* cbct, float
         } else {
             DISC_TRY(launch_upsample(c, c->lv[l + 1], c->lv[l + 1].disp, r, st));
         }
-        DISC_TRY(launch_moments<kModeZscore>(c, L, pcb[l], nullptr, L.zhat, nullptr, st));
+        DISC_TRY(launch_moments<kModeZscore>(c, L, pcb[l], nullptr, L.zhat, nullptr, kNoCtl, st));
         DISC_TRY(launch_warp(c, L, pct[l], r, L.m, st));
         const bool need_m = (l == 0 && out_corrected_cbct != nullptr);
         DISC_TRY(iterate_level(c, L, pct[l], r, c->iters, need_m, st));
         if (need_m)                                                                    // reading A12
-            DISC_TRY(launch_moments<kModeCorrect>(c, L, L.m, L.zhat, out_corrected_cbct, nullptr, st));
+            DISC_TRY(launch_moments<kModeCorrect>(c, L, L.m, L.zhat, out_corrected_cbct, nullptr, kNoCtl, st));
     }
     return DISC_OK;
 }
@@ -460,6 +421,7 @@ disc_status disc_register(disc_ctx* c, const float* ct, const float* cbct, float
 disc_status disc_register_host(disc_ctx* c, const float* ct_host, const float* cbct_host, float* out_disp_host,
                                float* out_corr_host, void* stream) {
     if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
     DISC_NEED(c, ct_host && cbct_host && out_disp_host, "NULL pointer");
     cudaStream_t st = (cudaStream_t)stream;
     const size_t b = c->lv[0].N * sizeof(float);
@@ -483,13 +445,15 @@ disc_status disc_register_host(disc_ctx* c, const float* ct_host, const float* c
 
 disc_status disc_box_moments(disc_ctx* c, int level, const float* vol, float* mean, float* var, void* stream) {
     if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
     DISC_NEED(c, level_ok(c, level), "level out of range");
     DISC_NEED(c, vol && mean && var, "NULL pointer");
-    return launch_moments<kModeMoments>(c, c->lv[level], vol, nullptr, mean, var, (cudaStream_t)stream);
+    return launch_moments<kModeMoments>(c, c->lv[level], vol, nullptr, mean, var, kNoCtl, (cudaStream_t)stream);
 }
 
 disc_status disc_force_update(disc_ctx* c, int level, const float* m, const float* s, float* disp_inout, void* stream) {
     if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
     DISC_NEED(c, level_ok(c, level), "level out of range");
     DISC_NEED(c, m && s && disp_inout, "NULL pointer");
     const Level& L = c->lv[level];
@@ -499,16 +463,18 @@ disc_status disc_force_update(disc_ctx* c, int level, const float* m, const floa
 
 disc_status disc_smooth_field(disc_ctx* c, int level, float* disp_inout, void* stream) {
     if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
     DISC_NEED(c, level_ok(c, level), "level out of range");
     DISC_NEED(c, disp_inout, "NULL pointer");
     Level& L = c->lv[level];
     cudaStream_t st = (cudaStream_t)stream;
-    DISC_TRY(launch_force_gxy(c, false, L, nullptr, nullptr, disp_inout, L.scratch, st));
-    return launch_gz_warp<false>(c, L, L.scratch, disp_inout, nullptr, nullptr, st);
+    DISC_TRY(launch_force_gxy(c, false, L, nullptr, nullptr, disp_inout, L.scratch, kNoCtl, st));
+    return launch_gz_warp<false>(c, L, L.scratch, disp_inout, nullptr, nullptr, kNoCtl, st);
 }
 
 disc_status disc_downsample(disc_ctx* c, int level_from, const float* vol, float* out, void* stream) {
     if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
     DISC_NEED(c, level_from >= 0 && level_from + 1 < c->levels, "level_from out of range");
     DISC_NEED(c, vol && out, "NULL pointer");
     return launch_downsample(c, c->lv[level_from], vol, out, (cudaStream_t)stream);
@@ -516,6 +482,7 @@ disc_status disc_downsample(disc_ctx* c, int level_from, const float* vol, float
 
 disc_status disc_upsample_field(disc_ctx* c, int level_from, const float* disp, float* out, void* stream) {
     if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
     DISC_NEED(c, level_from >= 1 && level_from < c->levels, "level_from out of range");
     DISC_NEED(c, disp && out, "NULL pointer");
     return launch_upsample(c, c->lv[level_from], disp, out, (cudaStream_t)stream);

@@ -229,8 +229,7 @@ k_warp(const float* __restrict__ moving, const float* __restrict__ r, float* __r
     if (x >= nx) return;
     const size_t N = (size_t)nx * ny * nz;
     const size_t i = ((size_t)z * ny + y) * nx + x;
-    out[i] = trilinear_clamped(moving, nx, ny, nz, (float)x + __ldg(r + i), (float)y + __ldg(r + N + i),
-                               (float)z + __ldg(r + 2 * N + i));
+    out[i] = trilinear_at_voxel(moving, nx, ny, nz, x, y, z, __ldg(r + i), __ldg(r + N + i), __ldg(r + 2 * N + i));
 }
 
 }  // namespace disc

@@ -13,78 +13,85 @@ namespace disc {
 
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+static int pick_chunk(int n, int min_chunk, long long ctas_per_chunk, long long target_ctas) {
+    // split an axis of length n into chunks so that the grid reaches ~target_ctas CTAs,
+    // but never below min_chunk (each chunk re-reads a halo)
+    long long want = target_ctas / ctas_per_chunk;  // round down: prefer one full wave over 1.x waves
+    if (want < 1) want = 1;
+    int chunk = (int)((n + want - 1) / want);
+    if (chunk < min_chunk) chunk = min_chunk;
+    if (chunk > n) chunk = n;
+    return chunk;
+}
+
 template <int K, int FORCE>
-static void launch_fg(int txb, const float* m, const float* s, const float* rin, float* rout, int nx, int ny, int nz,
-                      int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
+static void launch_fg(const DevInfo& di, const float* m, const float* s, const float* rin, float* rout, int nx, int ny,
+                      int nz, float eps_den, const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
     const bool vec_ok = nx % 4 == 0 && aligned16(rin) && aligned16(rout) && (!FORCE || (aligned16(m) && aligned16(s))) &&
                         3ull * nx * ny * nz < 0xffffffffull;   // the tile kernel indexes voxels with 32 bits
-    static int n_sm = 0;
-    if (!n_sm) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-    }
-    if (vec_ok) {
+    const int n_sm = di.n_sm;
+    if (vec_ok && di.dev >= 0 && di.dev < kMaxDevices) {
         using C = FgT4Cfg<K>;
-        static bool configured = false;  // one attribute call per instance (idempotent, so a race is harmless)
-        if (!configured) {
+        static bool configured[kMaxDevices] = {};  // the opt-in is per device (idempotent, so a race is harmless)
+        if (!configured[di.dev]) {
             cudaFuncSetAttribute(k_force_gxy_t4<K, FORCE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
-            configured = true;
+            configured[di.dev] = true;
         }
         const long long n_tiles = (long long)((nx + C::TX - 1) / C::TX) * ((ny + C::TY - 1) / C::TY) * nz;
         const int grid = (int)(n_tiles < (long long)C::OCC * n_sm ? n_tiles : (long long)C::OCC * n_sm);   // persistent: OCC CTAs per SM
-        k_force_gxy_t4<K, FORCE><<<grid, C::NT, C::smem_bytes, st>>>(m, s, rin, rout, nx, ny, nz, eps_den, taps, g_iter_ctl);
+        k_force_gxy_t4<K, FORCE><<<grid, C::NT, C::smem_bytes, st>>>(m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl);
         return;
     }
+    const int txb = nx > 64 ? 128 : (nx > 32 ? 64 : 32);
+    const int xt = (nx + txb - 1) / txb;
+    const int yseg = pick_chunk(ny, 8 * K > 32 ? 8 * K : 32, (long long)xt * nz, 4LL * n_sm);
     dim3 grid((nx + txb - 1) / txb, (ny + yseg - 1) / yseg, nz);
     if (txb == 128)
-        k_force_gxy<K, FORCE, 128><<<grid, 128, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, g_iter_ctl);
+        k_force_gxy<K, FORCE, 128><<<grid, 128, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, ctl);
     else if (txb == 64)
-        k_force_gxy<K, FORCE, 64><<<grid, 64, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, g_iter_ctl);
+        k_force_gxy<K, FORCE, 64><<<grid, 64, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, ctl);
     else
-        k_force_gxy<K, FORCE, 32><<<grid, 32, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, g_iter_ctl);
+        k_force_gxy<K, FORCE, 32><<<grid, 32, 0, st>>>(m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, ctl);
 }
 
 template <int K, bool WARP, int LZ>
 static void launch_gzd(const float* rin, float* rout, const float* moving, float* mout, int nx, int ny, int nz,
-                       const GaussTaps& taps, cudaStream_t st) {
+                       const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
     const size_t plane = (size_t)nx * ny;
     dim3 grid((unsigned)((plane + kGzdThreads - 1) / kGzdThreads), (nz + LZ - 1) / LZ, 1);
-    k_gz_warp_d<K, WARP, LZ><<<grid, kGzdThreads, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, taps, g_iter_ctl);
+    k_gz_warp_d<K, WARP, LZ><<<grid, kGzdThreads, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, taps, ctl);
 }
 
 template <int K, bool WARP, int LZ>
 static void launch_gzd2(const float* rin, float* rout, const float* moving, float* mout, int nx, int ny, int nz,
-                        const GaussTaps& taps, cudaStream_t st) {
+                        const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
     const size_t pairs = (size_t)nx * ny / 2;
     dim3 grid((unsigned)((pairs + kGzdThreads - 1) / kGzdThreads), (nz + LZ - 1) / LZ, 1);
-    k_gz_warp_d2<K, WARP, LZ><<<grid, kGzdThreads, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, taps, g_iter_ctl);
+    k_gz_warp_d2<K, WARP, LZ><<<grid, kGzdThreads, 0, st>>>(rin, rout, moving, mout, nx, ny, nz, taps, ctl);
 }
 
 static inline bool aligned8(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 7u) == 0; }
 
+// A thread owns two adjacent columns (one when nx is odd or a field is not 8-byte aligned) and 4 output slices;
+// measured on B200: with two columns per thread 4 slices beat 8 at every level (more threads in flight; the 2K
+// halo re-reads come from L2).
 template <int K, bool WARP>
 static void launch_gz(const float* rin, float* rout, const float* moving, float* mout, int nx, int ny, int nz,
-                      int zchunk, const GaussTaps& taps, cudaStream_t st) {
-    // zchunk = output slices per thread (4 or 8) + 100 * (columns per thread, 1 or 2), chosen by the caller
-    const int lz = zchunk % 100, two = zchunk / 100 >= 2;
-    if (two && nx % 2 == 0 && aligned8(rin) && aligned8(rout) && (!WARP || aligned8(mout))) {
-        if (lz >= 8) launch_gzd2<K, WARP, 8>(rin, rout, moving, mout, nx, ny, nz, taps, st);
-        else launch_gzd2<K, WARP, 4>(rin, rout, moving, mout, nx, ny, nz, taps, st);
-        return;
-    }
-    if (lz >= 8) launch_gzd<K, WARP, 8>(rin, rout, moving, mout, nx, ny, nz, taps, st);
-    else launch_gzd<K, WARP, 4>(rin, rout, moving, mout, nx, ny, nz, taps, st);
+                      const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
+    if (nx % 2 == 0 && aligned8(rin) && aligned8(rout) && (!WARP || aligned8(mout)))
+        launch_gzd2<K, WARP, 4>(rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
+    else
+        launch_gzd<K, WARP, 4>(rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
 }
 
 // one Gaussian radius: launches if K lies in this unit's range (the discarded branch is never instantiated)
 template <int K>
-static bool case_fg(int force, int txb, const float* m, const float* s, const float* rin, float* rout, int nx, int ny,
-                    int nz, int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
+static bool case_fg(const DevInfo& di, int force, const float* m, const float* s, const float* rin, float* rout, int nx,
+                    int ny, int nz, float eps_den, const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
     if constexpr (K >= DISC_K_LO && K <= DISC_K_HI) {
-        if (force == kForceDouble) launch_fg<K, kForceDouble>(txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
-        else if (force == kForceSingle) launch_fg<K, kForceSingle>(txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
-        else launch_fg<K, kForceNone>(txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
+        if (force == kForceDouble) launch_fg<K, kForceDouble>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
+        else if (force == kForceSingle) launch_fg<K, kForceSingle>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
+        else launch_fg<K, kForceNone>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
         return true;
     } else {
         return false;
@@ -93,10 +100,10 @@ static bool case_fg(int force, int txb, const float* m, const float* s, const fl
 
 template <int K>
 static bool case_gz(bool warp, const float* rin, float* rout, const float* moving, float* mout, int nx, int ny, int nz,
-                    int zchunk, const GaussTaps& taps, cudaStream_t st) {
+                    const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
     if constexpr (K >= DISC_K_LO && K <= DISC_K_HI) {
-        if (warp) launch_gz<K, true>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st);
-        else launch_gz<K, false>(rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st);
+        if (warp) launch_gz<K, true>(rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
+        else launch_gz<K, false>(rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
         return true;
     } else {
         return false;
@@ -105,24 +112,25 @@ static bool case_gz(bool warp, const float* rin, float* rout, const float* movin
 
 #define DISC_FOR_K(X) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12)
 
-bool DISC_CAT(launch_force_gxy_tu, DISC_TU)(int K, int force, int txb, const float* m, const float* s,
-                                            const float* rin, float* rout, int nx, int ny, int nz, int yseg,
-                                            float eps_den, const GaussTaps& taps, cudaStream_t st) {
+bool DISC_CAT(launch_force_gxy_tu, DISC_TU)(const DevInfo& di, int K, int force, const float* m, const float* s,
+                                            const float* rin, float* rout, int nx, int ny, int nz, float eps_den,
+                                            const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
     switch (K) {
 #define DISC_CASE(k) \
-    case k: return case_fg<k>(force, txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
+    case k: return case_fg<k>(di, force, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
         DISC_FOR_K(DISC_CASE)
 #undef DISC_CASE
     }
     return false;
 }
 
-bool DISC_CAT(launch_gz_warp_tu, DISC_TU)(int K, bool warp, const float* rin, float* rout, const float* moving,
-                                          float* mout, int nx, int ny, int nz, int zchunk, const GaussTaps& taps,
-                                          cudaStream_t st) {
+bool DISC_CAT(launch_gz_warp_tu, DISC_TU)(const DevInfo& di, int K, bool warp, const float* rin, float* rout,
+                                          const float* moving, float* mout, int nx, int ny, int nz,
+                                          const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
+    (void)di;
     switch (K) {
 #define DISC_CASE(k) \
-    case k: return case_gz<k>(warp, rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st);
+    case k: return case_gz<k>(warp, rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
         DISC_FOR_K(DISC_CASE)
 #undef DISC_CASE
     }
@@ -163,28 +171,29 @@ void launch_warp_kernel(const float* moving, const float* r, float* out, int nx,
     k_warp<<<grid, 256, 0, st>>>(moving, r, out, nx, ny, nz);
 }
 
-bool launch_moments_any(int R, int mode, int ty, const float* vol, const float* aux, float* out0, float* out1, int nx,
-                        int ny, int nz, int zchunk, float eps_var, cudaStream_t st) {
-    return launch_moments_tu0(R, mode, ty, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st) ||
-           launch_moments_tu1(R, mode, ty, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st) ||
-           launch_moments_tu2(R, mode, ty, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st) ||
-           launch_moments_tu3(R, mode, ty, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st);
+bool launch_moments_any(const DevInfo& di, int rxy, int rz, int mode, const float* vol, const float* aux, float* out0,
+                        float* out1, int nx, int ny, int nz, float eps_var, IterCtl ctl, cudaStream_t st) {
+    return launch_moments_tu0(di, rxy, rz, mode, vol, aux, out0, out1, nx, ny, nz, eps_var, ctl, st) ||
+           launch_moments_tu1(di, rxy, rz, mode, vol, aux, out0, out1, nx, ny, nz, eps_var, ctl, st) ||
+           launch_moments_tu2(di, rxy, rz, mode, vol, aux, out0, out1, nx, ny, nz, eps_var, ctl, st) ||
+           launch_moments_tu3(di, rxy, rz, mode, vol, aux, out0, out1, nx, ny, nz, eps_var, ctl, st);
 }
 
-bool launch_force_gxy_any(int K, int force, int txb, const float* m, const float* s, const float* rin, float* rout,
-                          int nx, int ny, int nz, int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st) {
-    return launch_force_gxy_tu0(K, force, txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st) ||
-           launch_force_gxy_tu1(K, force, txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st) ||
-           launch_force_gxy_tu2(K, force, txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st) ||
-           launch_force_gxy_tu3(K, force, txb, m, s, rin, rout, nx, ny, nz, yseg, eps_den, taps, st);
+bool launch_force_gxy_any(const DevInfo& di, int K, int force, const float* m, const float* s, const float* rin,
+                          float* rout, int nx, int ny, int nz, float eps_den, const GaussTaps& taps, IterCtl ctl,
+                          cudaStream_t st) {
+    return launch_force_gxy_tu0(di, K, force, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st) ||
+           launch_force_gxy_tu1(di, K, force, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st) ||
+           launch_force_gxy_tu2(di, K, force, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st) ||
+           launch_force_gxy_tu3(di, K, force, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
 }
 
-bool launch_gz_warp_any(int K, bool warp, const float* rin, float* rout, const float* moving, float* mout, int nx,
-                        int ny, int nz, int zchunk, const GaussTaps& taps, cudaStream_t st) {
-    return launch_gz_warp_tu0(K, warp, rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st) ||
-           launch_gz_warp_tu1(K, warp, rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st) ||
-           launch_gz_warp_tu2(K, warp, rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st) ||
-           launch_gz_warp_tu3(K, warp, rin, rout, moving, mout, nx, ny, nz, zchunk, taps, st);
+bool launch_gz_warp_any(const DevInfo& di, int K, bool warp, const float* rin, float* rout, const float* moving,
+                        float* mout, int nx, int ny, int nz, const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
+    return launch_gz_warp_tu0(di, K, warp, rin, rout, moving, mout, nx, ny, nz, taps, ctl, st) ||
+           launch_gz_warp_tu1(di, K, warp, rin, rout, moving, mout, nx, ny, nz, taps, ctl, st) ||
+           launch_gz_warp_tu2(di, K, warp, rin, rout, moving, mout, nx, ny, nz, taps, ctl, st) ||
+           launch_gz_warp_tu3(di, K, warp, rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
 }
 #endif
 

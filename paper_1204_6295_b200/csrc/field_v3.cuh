@@ -27,17 +27,31 @@ struct TriSample {
     float tx, ty, tz;
 };
 
+// Cell and weight of one axis of the sample position p = clamp(i + r, 0, n - 1) (reading A11), WITHOUT forming i + r:
+// floor(i + r) = i + floor(r) and the weight r - floor(r) are exact in fp32, whereas fl(i + r) loses up to
+// ulp(i)/2 = 3e-5 voxel at i ~ 500 -- at a 1000 HU/voxel edge that is 0.03 HU of the warped image, the largest
+// single term of the whole-schedule field error before this change (profiles/r02_accuracy.md).
+// p < 0 -> cell 0, weight 0; p >= n - 1 -> cell n - 2, weight 1 (n >= 2).
+__device__ __forceinline__ void tri_axis(int i, float r, int n, int& i0, float& t) {
+    const float fl = floorf(r);
+    i0 = i + (int)fl;
+    t = r - fl;
+    const bool lo = i0 < 0, hi = i0 > n - 2;
+    i0 = lo ? 0 : (hi ? n - 2 : i0);
+    t = lo ? 0.f : (hi ? 1.f : t);
+}
+
 // FAST: every axis has at least two voxels (checked once per kernel, uniform), so the neighbour offsets are the
-// constants +1, +nx, +plane and the eight addresses share four row pointers.
+// constants +1, +nx, +plane and the eight addresses share four row pointers.  (x, y, z): the voxel, (rx, ry, rz): its
+// displacement.
 template <bool FAST>
-__device__ __forceinline__ void tri_issue(const float* __restrict__ I, int nx, int ny, int nz, float px, float py,
-                                          float pz, TriSample& s) {
-    px = fminf(fmaxf(px, 0.f), (float)(nx - 1));
-    py = fminf(fmaxf(py, 0.f), (float)(ny - 1));
-    pz = fminf(fmaxf(pz, 0.f), (float)(nz - 1));
+__device__ __forceinline__ void tri_issue(const float* __restrict__ I, int nx, int ny, int nz, int x, int y, int z,
+                                          float rx, float ry, float rz, TriSample& s) {
     if (FAST) {
-        const int x0 = min((int)px, nx - 2), y0 = min((int)py, ny - 2), z0 = min((int)pz, nz - 2);
-        s.tx = px - (float)x0; s.ty = py - (float)y0; s.tz = pz - (float)z0;
+        int x0, y0, z0;
+        tri_axis(x, rx, nx, x0, s.tx);
+        tri_axis(y, ry, ny, y0, s.ty);
+        tri_axis(z, rz, nz, z0, s.tz);
         const float* p00 = I + ((size_t)(unsigned)((z0 * ny + y0) * nx + x0));
         const float* p10 = p00 + nx;
         const float* p01 = p00 + (size_t)nx * ny;
@@ -47,11 +61,14 @@ __device__ __forceinline__ void tri_issue(const float* __restrict__ I, int nx, i
         s.a[4] = __ldg(p01); s.a[5] = __ldg(p01 + 1);
         s.a[6] = __ldg(p11); s.a[7] = __ldg(p11 + 1);
     } else {
-        const int x0 = max(min((int)px, nx - 2), 0), y0 = max(min((int)py, ny - 2), 0), z0 = max(min((int)pz, nz - 2), 0);
+        int x0 = 0, y0 = 0, z0 = 0;
+        s.tx = 0.f; s.ty = 0.f; s.tz = 0.f;            // an axis of length 1 has weight 0
+        if (nx > 1) tri_axis(x, rx, nx, x0, s.tx);
+        if (ny > 1) tri_axis(y, ry, ny, y0, s.ty);
+        if (nz > 1) tri_axis(z, rz, nz, z0, s.tz);
         const int dx = nx > 1 ? 1 : 0;
         const int dy = ny > 1 ? nx : 0;
         const size_t dz = nz > 1 ? (size_t)nx * ny : 0;
-        s.tx = px - (float)x0; s.ty = py - (float)y0; s.tz = pz - (float)z0;
         const float* p = I + ((size_t)z0 * ny + y0) * nx + x0;
         s.a[0] = __ldg(p); s.a[1] = __ldg(p + dx);
         s.a[2] = __ldg(p + dy); s.a[3] = __ldg(p + dy + dx);
@@ -87,11 +104,11 @@ k_warp2(const float* __restrict__ moving, const float* __restrict__ r, float* __
     const bool fast = nx > 1 && ny > 1 && nz > 1 && N < (size_t)0x7fffffff;   // 32-bit voxel indices
     TriSample g0, g1;
     if (fast) {
-        tri_issue<true>(moving, nx, ny, nz, (float)x + rx.x, (float)y + ry.x, (float)z + rz.x, g0);
-        tri_issue<true>(moving, nx, ny, nz, (float)(x + 1) + rx.y, (float)y + ry.y, (float)z + rz.y, g1);
+        tri_issue<true>(moving, nx, ny, nz, x, y, z, rx.x, ry.x, rz.x, g0);
+        tri_issue<true>(moving, nx, ny, nz, x + 1, y, z, rx.y, ry.y, rz.y, g1);
     } else {
-        tri_issue<false>(moving, nx, ny, nz, (float)x + rx.x, (float)y + ry.x, (float)z + rz.x, g0);
-        tri_issue<false>(moving, nx, ny, nz, (float)(x + 1) + rx.y, (float)y + ry.y, (float)z + rz.y, g1);
+        tri_issue<false>(moving, nx, ny, nz, x, y, z, rx.x, ry.x, rz.x, g0);
+        tri_issue<false>(moving, nx, ny, nz, x + 1, y, z, rx.y, ry.y, rz.y, g1);
     }
     *reinterpret_cast<float2*>(out + i) = make_float2(tri_finish(g0), tri_finish(g1));
 }
@@ -143,7 +160,6 @@ k_gz_warp_d(const float* __restrict__ rin, float* __restrict__ rout, const float
     }
     if (WARP) {
         const int y = (int)(col / (unsigned)nx), x = (int)(col - (unsigned)y * (unsigned)nx);
-        const float fx = (float)x, fy = (float)y;
         const bool fast = nx > 1 && ny > 1 && nz > 1 && N < (size_t)0x7fffffff;   // 32-bit voxel indices
         float* mp = mout + (size_t)z0 * plane + col;
         constexpr int B = 4;
@@ -154,9 +170,8 @@ k_gz_warp_d(const float* __restrict__ rin, float* __restrict__ rout, const float
 #pragma unroll
             for (int b = 0; b < B; ++b) {
                 const int j = j0 + b;
-                const float fz = (float)(z0 + j);
-                if (fast) tri_issue<true>(moving, nx, ny, nz, fx + res[0][j], fy + res[1][j], fz + res[2][j], g[b]);
-                else tri_issue<false>(moving, nx, ny, nz, fx + res[0][j], fy + res[1][j], fz + res[2][j], g[b]);
+                if (fast) tri_issue<true>(moving, nx, ny, nz, x, y, z0 + j, res[0][j], res[1][j], res[2][j], g[b]);
+                else tri_issue<false>(moving, nx, ny, nz, x, y, z0 + j, res[0][j], res[1][j], res[2][j], g[b]);
             }
 #pragma unroll
             for (int b = 0; b < B; ++b) {
@@ -213,13 +228,9 @@ k_gz_warp_d2(const float* __restrict__ rin, float* __restrict__ rout, const floa
     }
     if (WARP) {
         const int y = (int)(col / (unsigned)nx), x = (int)(col - (unsigned)y * (unsigned)nx);   // both columns share y (nx even)
-        const float fx0 = (float)x, fx1 = (float)(x + 1), fy = (float)y;
         const bool fast = nx > 1 && ny > 1 && nz > 1 && N < (size_t)0x7fffffff;   // 32-bit voxel indices
         float* mp = mout + (size_t)z0 * plane + col;
-#ifndef DISC_GZ_B
-#define DISC_GZ_B 1
-#endif
-        constexpr int B = DISC_GZ_B;
+        constexpr int B = 1;   // gather batches of one slice (two voxels, 16 loads in flight) measured best
         static_assert(LZ % B == 0, "gather batches");
 #pragma unroll
         for (int j0 = 0; j0 < LZ; j0 += B) {
@@ -227,13 +238,12 @@ k_gz_warp_d2(const float* __restrict__ rin, float* __restrict__ rout, const floa
 #pragma unroll
             for (int b = 0; b < B; ++b) {
                 const int j = j0 + b;
-                const float fz = (float)(z0 + j);
                 if (fast) {
-                    tri_issue<true>(moving, nx, ny, nz, fx0 + res[0][j].x, fy + res[1][j].x, fz + res[2][j].x, g[b][0]);
-                    tri_issue<true>(moving, nx, ny, nz, fx1 + res[0][j].y, fy + res[1][j].y, fz + res[2][j].y, g[b][1]);
+                    tri_issue<true>(moving, nx, ny, nz, x, y, z0 + j, res[0][j].x, res[1][j].x, res[2][j].x, g[b][0]);
+                    tri_issue<true>(moving, nx, ny, nz, x + 1, y, z0 + j, res[0][j].y, res[1][j].y, res[2][j].y, g[b][1]);
                 } else {
-                    tri_issue<false>(moving, nx, ny, nz, fx0 + res[0][j].x, fy + res[1][j].x, fz + res[2][j].x, g[b][0]);
-                    tri_issue<false>(moving, nx, ny, nz, fx1 + res[0][j].y, fy + res[1][j].y, fz + res[2][j].y, g[b][1]);
+                    tri_issue<false>(moving, nx, ny, nz, x, y, z0 + j, res[0][j].x, res[1][j].x, res[2][j].x, g[b][0]);
+                    tri_issue<false>(moving, nx, ny, nz, x + 1, y, z0 + j, res[0][j].y, res[1][j].y, res[2][j].y, g[b][1]);
                 }
             }
 #pragma unroll

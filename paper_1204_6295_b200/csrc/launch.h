@@ -10,7 +10,13 @@
 namespace disc {
 
 constexpr int kMomTX = 32, kMomTY = 16;  // (x,y) tile of the plain-load moments kernel
-constexpr int kMomMaxRTile32 = 7;        // largest R whose z ring fits tensor memory with the 32x32 tile (moments_v2.cuh)
+constexpr int kMaxDevices = 64;          // per-device "attribute set" flags of the launchers
+
+// What a launcher needs to know about the context's device (set in disc_create).
+struct DevInfo {
+    int dev;    // CUDA device ordinal the context lives on
+    int n_sm;   // its multiprocessor count
+};
 
 enum MomentsMode {
     kModeMoments = 0,  // out0 = mean, out1 = var                                   (disc_box_moments)
@@ -18,36 +24,36 @@ enum MomentsMode {
     kModeCorrect = 2   // out0 = sigma_m * aux + mu_m  (aux = CBCT z-score)          (per-iteration correction)
 };
 
-
-// Stop control handed to every kernel launched from this host thread ({nullptr, 0}: criterion off); set by
-// disc_api.cu around the launches of one iteration.
-extern thread_local IterCtl g_iter_ctl;
 // sum|dr|, sum|r| of the iteration -> l^(k), criterion check in the last block (field.cuh k_force_norms)
 void launch_force_norms(int force, const float* m, const float* s, const float* r, int nx, int ny, int nz, float eps_den,
                         StopCtl* ctl, int iter, float stop_eps, int n_sm, cudaStream_t st);
 void launch_stop_reset(StopCtl* ctl, cudaStream_t st);
 void launch_stop_record(StopCtl* ctl, int level, int n_iters, cudaStream_t st);
 
-bool launch_moments_any(int R, int mode, int ty, const float* vol, const float* aux, float* out0, float* out1, int nx,
-                        int ny, int nz, int zchunk, float eps_var, cudaStream_t st);
+// Every iteration kernel takes the stop control of its iteration by value ({nullptr, 0}: criterion off).
+// rxy: patch radius along x and y, rz: along z; zchunk <= 0: the launcher picks the z chunk.
+bool launch_moments_any(const DevInfo& di, int rxy, int rz, int mode, const float* vol, const float* aux, float* out0,
+                        float* out1, int nx, int ny, int nz, float eps_var, IterCtl ctl, cudaStream_t st);
 // force = 0 none (plain smoothing), 1 Thirion / passive, 2 double (ForceMode in field.cuh)
-bool launch_force_gxy_any(int K, int force, int txb, const float* m, const float* s, const float* rin, float* rout,
-                          int nx, int ny, int nz, int yseg, float eps_den, const GaussTaps& taps, cudaStream_t st);
-bool launch_gz_warp_any(int K, bool warp, const float* rin, float* rout, const float* moving, float* mout, int nx,
-                        int ny, int nz, int zchunk, const GaussTaps& taps, cudaStream_t st);
+bool launch_force_gxy_any(const DevInfo& di, int K, int force, const float* m, const float* s, const float* rin,
+                          float* rout, int nx, int ny, int nz, float eps_den, const GaussTaps& taps, IterCtl ctl,
+                          cudaStream_t st);
+bool launch_gz_warp_any(const DevInfo& di, int K, bool warp, const float* rin, float* rout, const float* moving,
+                        float* mout, int nx, int ny, int nz, const GaussTaps& taps, IterCtl ctl, cudaStream_t st);
 void launch_force_update(int force, const float* m, const float* s, float* r, int nx, int ny, int nz, float eps_den,
                          cudaStream_t st);
 void launch_warp_kernel(const float* moving, const float* r, float* out, int nx, int ny, int nz, cudaStream_t st);
 
 // per-translation-unit entry points (defined by moments_tu.cu / field_tu.cu with -DDISC_TU=n)
 #define DISC_DECL_TU(n)                                                                                                  \
-    bool launch_moments_tu##n(int R, int mode, int ty, const float* vol, const float* aux, float* out0, float* out1, int nx,     \
-                              int ny, int nz, int zchunk, float eps_var, cudaStream_t st);                              \
-    bool launch_force_gxy_tu##n(int K, int force, int txb, const float* m, const float* s, const float* rin,           \
-                                float* rout, int nx, int ny, int nz, int yseg, float eps_den, const GaussTaps& taps,    \
+    bool launch_moments_tu##n(const DevInfo& di, int rxy, int rz, int mode, const float* vol, const float* aux,         \
+                              float* out0, float* out1, int nx, int ny, int nz, float eps_var, IterCtl ctl,             \
+                              cudaStream_t st);                                                                          \
+    bool launch_force_gxy_tu##n(const DevInfo& di, int K, int force, const float* m, const float* s, const float* rin,  \
+                                float* rout, int nx, int ny, int nz, float eps_den, const GaussTaps& taps, IterCtl ctl, \
                                 cudaStream_t st);                                                                        \
-    bool launch_gz_warp_tu##n(int K, bool warp, const float* rin, float* rout, const float* moving, float* mout,        \
-                              int nx, int ny, int nz, int zchunk, const GaussTaps& taps, cudaStream_t st);
+    bool launch_gz_warp_tu##n(const DevInfo& di, int K, bool warp, const float* rin, float* rout, const float* moving,  \
+                              float* mout, int nx, int ny, int nz, const GaussTaps& taps, IterCtl ctl, cudaStream_t st);
 DISC_DECL_TU(0) DISC_DECL_TU(1) DISC_DECL_TU(2) DISC_DECL_TU(3)
 #undef DISC_DECL_TU
 

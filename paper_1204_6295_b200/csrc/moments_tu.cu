@@ -1,8 +1,8 @@
-// moments_tu.cu -- instantiates k_moments<R, MODE> for R in [DISC_R_LO, DISC_R_HI]; built once per range
+// moments_tu.cu -- instantiates k_moments_v3<R, TY, MODE> and the plain-load k_moments<R, MODE> for R in [DISC_R_LO, DISC_R_HI]; built once per range
 // (-DDISC_TU=n -DDISC_R_LO=a -DDISC_R_HI=b) so the instances compile in parallel.
 #include "launch.h"
 #include "moments.cuh"
-#include "moments_v2.cuh"
+#include "moments_v3.cuh"
 
 #define DISC_CAT2(a, b) a##b
 #define DISC_CAT(a, b) DISC_CAT2(a, b)
@@ -26,36 +26,50 @@ static EncodeTiledFn encode_tiled() {
     return fn;
 }
 
+// z chunk of the marching kernels: minimise (waves of CTAs) x (slices marched per CTA, with the 2 rz halo and a few
+// slices of pipeline fill).  `slots` = CTAs resident on the device at once.
+static int pick_zchunk(long long tiles, long long slots, int nz, int rz) {
+    double best = 1e300;
+    int best_zc = nz;
+    for (int nchunk = 1; nchunk <= nz; ++nchunk) {
+        const int zc = (nz + nchunk - 1) / nchunk;
+        const long long ctas = tiles * ((nz + zc - 1) / zc);
+        const long long waves = (ctas + slots - 1) / slots;
+        const double cost = (double)waves * (zc + 2 * rz + 4);
+        if (cost < best) { best = cost; best_zc = zc; }
+        if (zc == 1) break;
+    }
+    return best_zc;
+}
+
 template <int R, int TY>
-static bool launch_r_v2(int mode, const float* vol, const float* aux, float* out0, float* out1, int nx, int ny,
-                        int nz, int zchunk, float eps_var, cudaStream_t st) {
-    using C = MomV2Cfg<R, TY>;
+static bool launch_r_v3(const DevInfo& di, int rz, int mode, const float* vol, const float* aux, float* out0,
+                        float* out1, int nx, int ny, int nz, float eps_var, IterCtl ctl, cudaStream_t st) {
+    using C = MomV3Cfg<R, TY>;
     EncodeTiledFn enc = encode_tiled();
     if (!enc) return false;
-    CUtensorMap tmap, tmap_aux;
+    CUtensorMap tmap;
     const cuuint64_t gdim[3] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz};
     const cuuint64_t gstr[2] = {(cuuint64_t)nx * 4, (cuuint64_t)nx * ny * 4};
     const cuuint32_t box[3] = {(cuuint32_t)C::PXB, (cuuint32_t)C::PY, 1};
-    const cuuint32_t box_aux[3] = {(cuuint32_t)C::TX, (cuuint32_t)TY, 1};
     const cuuint32_t estr[3] = {1, 1, 1};
-    // per-voxel operand of the evaluation: the volume itself (z-score), the cached z-score (correction)
-    const float* per_voxel = mode == kModeCorrect ? aux : vol;
     if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(vol), gdim, gstr, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS ||
-        enc(&tmap_aux, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(per_voxel), gdim, gstr, box_aux, estr,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return false;
-    static bool configured[3] = {false, false, false};
+    // per-voxel operand of the evaluation: the volume itself (z-score), the cached z-score (correction)
+    const float* pv = mode == kModeCorrect ? aux : vol;
+    const long long tiles = (long long)((nx + C::TX - 1) / C::TX) * ((ny + TY - 1) / TY);
+    const int zchunk = pick_zchunk(tiles, di.n_sm, nz, rz);
     dim3 grid((nx + C::TX - 1) / C::TX, (ny + TY - 1) / TY, (nz + zchunk - 1) / zchunk);
-#define DISC_LAUNCH_MODE(M)                                                                                         \
-    {                                                                                                               \
-        if (!configured[M]) {                                                                                       \
-            cudaFuncSetAttribute(k_moments_v2<R, TY, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes); \
-            configured[M] = true;                                                                                   \
-        }                                                                                                           \
-        k_moments_v2<R, TY, M><<<grid, C::NT, C::smem_bytes, st>>>(tmap, tmap_aux, out0, out1, nx, ny, nz, zchunk, eps_var, g_iter_ctl); \
+    static bool configured[3][kMaxDevices] = {};
+#define DISC_LAUNCH_MODE(M)                                                                                              \
+    {                                                                                                                    \
+        if (!configured[M][di.dev]) {   /* the opt-in is per device */                                                   \
+            cudaFuncSetAttribute(k_moments_v3<R, TY, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes); \
+            configured[M][di.dev] = true;                                                                                \
+        }                                                                                                                \
+        k_moments_v3<R, TY, M><<<grid, C::NT, C::smem_bytes, st>>>(tmap, pv, out0, out1, nx, ny, nz, rz, zchunk, eps_var, ctl); \
     }
     if (mode == kModeMoments) DISC_LAUNCH_MODE(kModeMoments)
     else if (mode == kModeZscore) DISC_LAUNCH_MODE(kModeZscore)
@@ -64,53 +78,66 @@ static bool launch_r_v2(int mode, const float* vol, const float* aux, float* out
     return true;
 }
 
+// the TMA kernel with the tile height the z window allows: 32 rows while the ring of 2 rz + 1 slots fits tensor
+// memory, 16 rows beyond (possible only when the tile + halo still has 32 rows, R >= 8)
 template <int R>
-static bool launch_r_tma(int mode, int ty, const float* vol, const float* aux, float* out0, float* out1, int nx,
-                         int ny, int nz, int zchunk, float eps_var, cudaStream_t st) {
-    if constexpr (R <= kMomMaxRTile32) {
-        if (ty == 32) return launch_r_v2<R, 32>(mode, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st);
+static bool launch_r_tma(const DevInfo& di, int rz, int mode, const float* vol, const float* aux, float* out0,
+                         float* out1, int nx, int ny, int nz, float eps_var, IterCtl ctl, cudaStream_t st) {
+    const int wz = 2 * rz + 1;
+    if (wz <= MomV3Cfg<R, 32>::WZ_MAX)
+        return launch_r_v3<R, 32>(di, rz, mode, vol, aux, out0, out1, nx, ny, nz, eps_var, ctl, st);
+    if constexpr (R >= 8) {
+        if (wz <= MomV3Cfg<R, 16>::WZ_MAX)
+            return launch_r_v3<R, 16>(di, rz, mode, vol, aux, out0, out1, nx, ny, nz, eps_var, ctl, st);
     }
-    return launch_r_v2<R, 16>(mode, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st);
+    return false;
 }
 
 template <int R>
-static void launch_r(int mode, int ty, const float* vol, const float* aux, float* out0, float* out1, int nx, int ny, int nz,
-                     int zchunk, float eps_var, cudaStream_t st) {
+static bool launch_r(const DevInfo& di, int rz, int mode, const float* vol, const float* aux, float* out0, float* out1,
+                     int nx, int ny, int nz, float eps_var, IterCtl ctl, cudaStream_t st) {
+    if (di.dev < 0 || di.dev >= kMaxDevices) return false;
     // TMA path: rows must be 16-byte multiples and the base 16-byte aligned (tensor-map requirements)
     if (nx % 4 == 0 && (reinterpret_cast<uintptr_t>(vol) & 15u) == 0 &&
-        (mode != kModeCorrect || (reinterpret_cast<uintptr_t>(aux) & 15u) == 0) &&
-        launch_r_tma<R>(mode, ty, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st))
-        return;
-    dim3 grid((nx + kMomTX - 1) / kMomTX, (ny + kMomTY - 1) / kMomTY, (nz + zchunk - 1) / zchunk);
-    constexpr int NT = MomCfg<R>::NT;
-    if (mode == kModeMoments)
-        k_moments<R, kModeMoments><<<grid, NT, 0, st>>>(vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, g_iter_ctl);
-    else if (mode == kModeZscore)
-        k_moments<R, kModeZscore><<<grid, NT, 0, st>>>(vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, g_iter_ctl);
-    else
-        k_moments<R, kModeCorrect><<<grid, NT, 0, st>>>(vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, g_iter_ctl);
+        launch_r_tma<R>(di, rz, mode, vol, aux, out0, out1, nx, ny, nz, eps_var, ctl, st))
+        return true;
+    if constexpr (R <= 10) {
+        if (rz == R) {   // plain-load kernel: cubic patches, any nx
+            const long long tiles = (long long)((nx + kMomTX - 1) / kMomTX) * ((ny + kMomTY - 1) / kMomTY);
+            const int zchunk = pick_zchunk(tiles, 2LL * di.n_sm, nz, rz);
+            dim3 grid((nx + kMomTX - 1) / kMomTX, (ny + kMomTY - 1) / kMomTY, (nz + zchunk - 1) / zchunk);
+            constexpr int NT = MomCfg<R>::NT;
+            if (mode == kModeMoments)
+                k_moments<R, kModeMoments><<<grid, NT, 0, st>>>(vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, ctl);
+            else if (mode == kModeZscore)
+                k_moments<R, kModeZscore><<<grid, NT, 0, st>>>(vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, ctl);
+            else
+                k_moments<R, kModeCorrect><<<grid, NT, 0, st>>>(vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, ctl);
+            return true;
+        }
+    }
+    return false;
 }
 
 // one radius: launches if R lies in this unit's range (the discarded branch is never instantiated)
 template <int R>
-static bool case_r(int mode, int ty, const float* vol, const float* aux, float* out0, float* out1, int nx, int ny,
-                   int nz, int zchunk, float eps_var, cudaStream_t st) {
+static bool case_r(const DevInfo& di, int rz, int mode, const float* vol, const float* aux, float* out0, float* out1,
+                   int nx, int ny, int nz, float eps_var, IterCtl ctl, cudaStream_t st) {
     if constexpr (R >= DISC_R_LO && R <= DISC_R_HI) {
-        launch_r<R>(mode, ty, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st);
-        return true;
+        return launch_r<R>(di, rz, mode, vol, aux, out0, out1, nx, ny, nz, eps_var, ctl, st);
     } else {
         return false;
     }
 }
 
-bool DISC_CAT(launch_moments_tu, DISC_TU)(int R, int mode, int ty, const float* vol, const float* aux,
-                                          float* out0, float* out1, int nx, int ny, int nz, int zchunk,
-                                          float eps_var, cudaStream_t st) {
-    switch (R) {
+bool DISC_CAT(launch_moments_tu, DISC_TU)(const DevInfo& di, int rxy, int rz, int mode, const float* vol,
+                                          const float* aux, float* out0, float* out1, int nx, int ny, int nz,
+                                          float eps_var, IterCtl ctl, cudaStream_t st) {
+    switch (rxy) {
 #define DISC_CASE(r) \
-    case r: return case_r<r>(mode, ty, vol, aux, out0, out1, nx, ny, nz, zchunk, eps_var, st);
-        DISC_CASE(0) DISC_CASE(1) DISC_CASE(2) DISC_CASE(3) DISC_CASE(4) DISC_CASE(5)
-        DISC_CASE(6) DISC_CASE(7) DISC_CASE(8) DISC_CASE(9) DISC_CASE(10)
+    case r: return case_r<r>(di, rz, mode, vol, aux, out0, out1, nx, ny, nz, eps_var, ctl, st);
+        DISC_CASE(0) DISC_CASE(1) DISC_CASE(2) DISC_CASE(3) DISC_CASE(4) DISC_CASE(5) DISC_CASE(6)
+        DISC_CASE(7) DISC_CASE(8) DISC_CASE(9) DISC_CASE(10) DISC_CASE(11) DISC_CASE(12)
 #undef DISC_CASE
     }
     return false;

@@ -24,6 +24,16 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+// Arrive that cannot be issued before `dep0` has been computed.  A consumer releases a buffer with it: shared-memory
+// loads still in flight when the producer overwrites the buffer are a race (seen on B200 with a plain arrive right
+// after the loads), and an arrive without a register dependency may be scheduled ahead of the instructions that
+// consume the loaded values.  dep0 = (a register computed from ALL loaded values) & (a run-time zero the compiler
+// cannot fold, see rt_zero()); it is added to the barrier address.
+__device__ __forceinline__ void mbar_arrive_after(uint64_t* bar, uint32_t dep0) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar) + dep0) : "memory");
+}
+// 0 for every legal volume (n < 2^30), opaque to the compiler
+__device__ __forceinline__ uint32_t rt_zero(int n) { return (uint32_t)n >> 30; }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     asm volatile(
         "{\n\t"

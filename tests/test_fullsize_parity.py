@@ -1,11 +1,11 @@
 """Parity at BASELINE.json's full size, in the launch configuration bench.py times: config 3 (256x256x128, R = 5,
 sigma = 2.0) and the largest single level of config 4 (512x512x128, R = 7) through the same C-ABI calls.
 
-The naive oracle needs ~4 s per full-size correction (16 cores), so: the cheap steps (warp, force + update,
-Gaussian) are compared element by element on the whole volume; the patch moments / correction on sampled voxels
-the oracle computes one by one (corners, edges, faces, tile seams and random interior points); two whole
-iterations of config 3's finest level element by element; and the whole 3 x 100 schedule through properties
-that hold at any size (reading A12 identity, the AM-GM bound of the force, image mismatch reduced).
+Every kernel is compared with the naive oracle element by element on the WHOLE volume (the patch moments and the
+correction too: ~3 s at config 3, ~25 s at config 4's finest level on the box's 16 cores), two whole iterations of
+config 3's finest level likewise, and the whole 3 x 100 schedule of config 3 -- the workload bench.py times --
+against oracle.register at north_star's 1e-2 voxel (~2 min of oracle time).  Config 4's 4 x 100 schedule is in
+tests/test_zz_config4_schedule.py.
 """
 import numpy as np
 import pytest
@@ -64,17 +64,20 @@ def test_config3_per_kernel_full_volume(disc, oracle_mod, pair3):
     disc.disc_warp(ctx, 0, d_ct, d_r0, d_m)
     m = d_m.cpu().numpy()
     assert np.abs(m - oracle_mod.warp(ct, r0)).max() <= 1e-4 * span
-    # correction and moments: sampled voxels, computed one by one by the naive oracle
-    idx = sample_indices(ct.shape, rng)
+    # correction and moments: EVERY voxel against the naive patch loops (PAPER.md:95 Eq. 3, :117-119 Eqs. 5-6)
     d_sp = torch.empty_like(d_ct)
     disc.disc_correct_intensity(ctx, 0, d_cb, d_m, d_sp)
     sp = d_sp.cpu().numpy()
-    assert np.abs(sp.ravel()[idx] - oracle_mod.correct_at(cbct, m, R, idx)).max() <= 1e-4 * span
+    mu_s, var_s = oracle_mod.box_moments(cbct, R)
+    mu_m, var_m = oracle_mod.box_moments(m, R)
+    assert np.abs(sp - oracle_mod.correct_from_moments(cbct, mu_s, var_s, mu_m, var_m)).max() <= 1e-4 * span
     d_mu, d_var = torch.empty_like(d_ct), torch.empty_like(d_ct)
     disc.disc_box_moments(ctx, 0, d_cb, d_mu, d_var)
-    mu_ref, var_ref = oracle_mod.box_moments_at(cbct, R, idx)
-    assert np.abs(d_mu.cpu().numpy().ravel()[idx] - mu_ref).max() <= 1e-4 * span
-    assert np.abs(np.sqrt(d_var.cpu().numpy().ravel()[idx]) - np.sqrt(var_ref)).max() <= 1e-4 * span
+    assert np.abs(d_mu.cpu().numpy() - mu_s).max() <= 1e-4 * span
+    assert np.abs(np.sqrt(d_var.cpu().numpy()) - np.sqrt(var_s)).max() <= 1e-4 * span
+    # the sampler agrees with the whole-volume loop at the seams (it is pinned on CPU, tests/test_oracle_pins_ext.py)
+    idx = sample_indices(ct.shape, rng, 50)
+    assert np.array_equal(oracle_mod.box_moments_at(cbct, R, idx)[0], mu_s.ravel()[idx])
     # force + update, Gaussian, demons step: whole volume (same fp32 inputs on both sides)
     d_r = d_r0.clone()
     disc.disc_force_update(ctx, 0, d_m, d_sp, d_r)
@@ -106,10 +109,15 @@ def test_config3_two_whole_iterations(disc, oracle_mod, pair3):
     assert err <= 1e-3, err
 
 
-def test_config3_whole_schedule_properties(disc, oracle_mod, pair3):
+@pytest.mark.slow
+def test_config3_whole_schedule_against_the_oracle(disc, oracle_mod, pair3):
+    """north_star: "final displacement within 1e-2 voxel max-abs after the full schedule" on the benchmarked workload:
+    256x256x128, 3 levels x 100 iterations, R = 5, sigma = 2 (Alg. A1), disc_register against
+    oracle.register (naive patch loops throughout, ~2 min on 16 cores)."""
     ct, cbct, u, p = pair3
     nz, ny, nx = ct.shape
     R, sigma = p["patch_radius"], p["sigma"]
+    assert (nx, ny, nz, R, p["levels"], p["iters"]) == (256, 256, 128, 5, 3, 100)
     ctx = disc.disc_create((nx, ny, nz), (1, 1, 1), R, sigma, p["levels"], p["iters"])
     d_ct, d_cb = dev(ct), dev(cbct)
     d_r, d_corr = torch.empty((3,) + ct.shape, device="cuda"), torch.empty_like(d_ct)
@@ -119,13 +127,15 @@ def test_config3_whole_schedule_properties(disc, oracle_mod, pair3):
     disc.disc_warp(ctx, 0, d_ct, d_r, d_m)
     disc.disc_correct_intensity(ctx, 0, d_cb, d_m, d_c2)
     assert torch.equal(d_c2, d_corr)
-    r = d_r.cpu().numpy()
+    r, corr, m = d_r.cpu().numpy(), d_corr.cpu().numpy(), d_m.cpu().numpy()
     assert np.isfinite(r).all()
-    # ... and it matches the naive oracle at sampled voxels
-    idx = sample_indices(ct.shape, np.random.default_rng(11), 200)
-    m = d_m.cpu().numpy()
+    r_ref, corr_ref = oracle_mod.register(ct, cbct, R, sigma, p["levels"], p["iters"])
+    err_r = float(np.abs(r - r_ref).max())
+    assert err_r <= 1e-2, f"field error {err_r} voxel after the 3 x 100 schedule"
     span = hu_range(ct, cbct)
-    assert np.abs(d_corr.cpu().numpy().ravel()[idx] - oracle_mod.correct_at(cbct, m, R, idx)).max() <= 1e-4 * span
+    g = float(np.abs(np.stack(np.gradient(ct.astype(np.float64)))).max())
+    err_c = float(np.abs(corr - corr_ref).max())
+    assert err_c <= 1e-4 * span + 2.0 * err_r * g + 1e-3, (err_c, err_r, g)
     # the registration did its job: the deformed CT is closer to the deformation-only target ct(x + u) than the CT
     target = phantoms.pullback(ct, u)
     body = target > -500.0
@@ -139,8 +149,9 @@ def test_config3_whole_schedule_properties(disc, oracle_mod, pair3):
     disc.disc_destroy(ctx)
 
 
-def test_config4_finest_level_sampled(disc, oracle_mod):
-    """512x512x128, R = 7 (patch 15^3), K = 6: correction at sampled voxels, field kernels on the whole volume"""
+@pytest.mark.slow
+def test_config4_finest_level_whole_volume(disc, oracle_mod):
+    """512x512x128, R = 7 (patch 15^3), K = 6: every kernel on the whole volume against the naive oracle"""
     dims, R, sigma = (512, 512, 128), 7, 2.0
     a, b, u = phantoms.make_sweep_inputs(dims, seed_offset=4)
     a = (a * 4.0).astype(np.float32)
@@ -151,45 +162,19 @@ def test_config4_finest_level_sampled(disc, oracle_mod):
     d_a, d_b, d_u = dev(a), dev(b), dev(u)
     d_sp = torch.empty_like(d_a)
     disc.disc_correct_intensity(ctx, 0, d_b, d_a, d_sp)
-    idx = sample_indices(a.shape, np.random.default_rng(13), 150)
     sp = d_sp.cpu().numpy()
-    assert np.abs(sp.ravel()[idx] - oracle_mod.correct_at(b, a, R, idx)).max() <= 1e-4 * span
+    mu_s, var_s = oracle_mod.box_moments(b, R)
+    mu_m, var_m = oracle_mod.box_moments(a, R)
+    assert np.abs(sp - oracle_mod.correct_from_moments(b, mu_s, var_s, mu_m, var_m)).max() <= 1e-4 * span
+    d_mu, d_var = torch.empty_like(d_a), torch.empty_like(d_a)
+    disc.disc_box_moments(ctx, 0, d_b, d_mu, d_var)
+    assert np.abs(d_mu.cpu().numpy() - mu_s).max() <= 1e-4 * span
+    assert np.abs(np.sqrt(d_var.cpu().numpy()) - np.sqrt(var_s)).max() <= 1e-4 * span
+    del mu_s, var_s, mu_m, var_m, d_mu, d_var
     d_r = d_u.clone()
     disc.disc_demons_step(ctx, 0, d_a, d_sp, d_r)
     assert np.abs(d_r.cpu().numpy() - oracle_mod.demons_step(a, sp, u, sigma)).max() <= 1e-4
     d_m = torch.empty_like(d_a)
     disc.disc_warp(ctx, 0, d_a, d_u, d_m)
     assert np.abs(d_m.cpu().numpy() - oracle_mod.warp(a, u)).max() <= 1e-4 * span
-    disc.disc_destroy(ctx)
-
-
-@pytest.mark.slow
-def test_config4_whole_schedule_properties(disc, oracle_mod):
-    """config 4 as BASELINE.json states it: 512x512x128, 4-level pyramid x 100 iterations, patch 15^3 (R = 7), sigma 2.
-    The naive oracle would need over an hour for this schedule, so the whole run is checked through properties that
-    hold at any size and through the oracle at sampled voxels of the returned corrected CBCT."""
-    ct, cbct, u, p = phantoms.make_pair(4)
-    nz, ny, nx = ct.shape
-    assert (nx, ny, nz) == (512, 512, 128) and p["patch_radius"] == 7 and p["levels"] == 4
-    R, sigma = p["patch_radius"], p["sigma"]
-    ctx = disc.disc_create((nx, ny, nz), (1, 1, 1), R, sigma, p["levels"], p["iters"])
-    d_ct, d_cb = dev(ct), dev(cbct)
-    d_r, d_corr = torch.empty((3,) + ct.shape, device="cuda"), torch.empty_like(d_ct)
-    disc.disc_register(ctx, d_ct, d_cb, d_r, d_corr)
-    assert disc.disc_iterations_run(ctx) == [p["iters"]] * p["levels"]
-    d_m, d_c2 = torch.empty_like(d_ct), torch.empty_like(d_ct)
-    disc.disc_warp(ctx, 0, d_ct, d_r, d_m)
-    disc.disc_correct_intensity(ctx, 0, d_cb, d_m, d_c2)
-    assert torch.equal(d_c2, d_corr)                                   # reading A12
-    assert bool(torch.isfinite(d_r).all())
-    m = d_m.cpu().numpy()
-    idx = sample_indices(ct.shape, np.random.default_rng(17), 120)
-    span = hu_range(ct, cbct)
-    assert np.abs(d_corr.cpu().numpy().ravel()[idx] - oracle_mod.correct_at(cbct, m, R, idx)).max() <= 1e-4 * span
-    assert np.abs(m - oracle_mod.warp(ct, d_r.cpu().numpy())).max() <= 1e-4 * span
-    target = phantoms.pullback(ct, u)
-    body = target > -500.0
-    rmse0 = np.sqrt(np.mean((ct - target)[body] ** 2))
-    rmse1 = np.sqrt(np.mean((m - target)[body] ** 2))
-    assert rmse1 < 0.7 * rmse0, (rmse0, rmse1)
     disc.disc_destroy(ctx)
