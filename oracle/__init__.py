@@ -34,7 +34,7 @@ _i64p = ctypes.POINTER(ctypes.c_longlong)
 def build(force: bool = False) -> str:
     """Compile the C oracle with gcc (-O2 -fopenmp).  Building the checker is not using it."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-o", _LIB, _SRC, "-lm"])
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=gnu99", "-o", _LIB, _SRC, "-lm"])
     return _LIB
 
 

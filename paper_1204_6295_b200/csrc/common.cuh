@@ -63,12 +63,13 @@ __device__ __forceinline__ float trilinear_clamped(const float* __restrict__ I, 
     return fmaf(tz, c1, uz * c0);
 }
 
-// The warp's sample m(x) = I(x + r(x)) with the cell and weights formed from the voxel's integer coordinate and its
-// displacement separately: floor(i + r) = i + floor(r) and r - floor(r) are exact in fp32 (fl(i + r) is not).
-// Per axis: p < 0 -> cell 0, weight 0; p >= n - 1 -> cell n - 2, weight 1; an axis of length 1 has weight 0.
+// The warp's sample m(x) = I(x + r(x)) with the cell and weight formed from the voxel's integer coordinate and its
+// displacement separately (floor(i + r) = i + floor(r) and r - floor(r) are exact in fp32, fl(i + r) is not) and the
+// lerp written a + t (b - a), b the neighbour at +1 inside the volume and at -1 for a sample clamped to the far face:
+// a zero field, an integer shift, a clamped sample and a flat region are all reproduced bit for bit (field_v3.cuh).
 __device__ __forceinline__ float trilinear_at_voxel(const float* __restrict__ I, int nx, int ny, int nz, int x, int y,
                                                     int z, float rx, float ry, float rz) {
-    int c0[3] = {0, 0, 0};
+    int c0[3] = {0, 0, 0}, st[3] = {0, 0, 0};
     float t[3] = {0.f, 0.f, 0.f};
     const int n[3] = {nx, ny, nz}, i[3] = {x, y, z};
     const float r[3] = {rx, ry, rz};
@@ -78,25 +79,24 @@ __device__ __forceinline__ float trilinear_at_voxel(const float* __restrict__ I,
             const float fl = floorf(r[a]);
             const int j = i[a] + (int)fl;
             const bool lo = j < 0, hi = j > n[a] - 2;
-            c0[a] = lo ? 0 : (hi ? n[a] - 2 : j);
-            t[a] = lo ? 0.f : (hi ? 1.f : r[a] - fl);
+            c0[a] = lo ? 0 : (hi ? n[a] - 1 : j);
+            t[a] = (lo || hi) ? 0.f : r[a] - fl;
+            st[a] = hi ? -1 : 1;
         }
     }
-    const int dx = nx > 1 ? 1 : 0;
-    const size_t dy = ny > 1 ? (size_t)nx : 0, dz = nz > 1 ? (size_t)nx * ny : 0;
+    const ptrdiff_t dx = st[0], dy = (ptrdiff_t)st[1] * nx, dz = (ptrdiff_t)st[2] * nx * ny;
     const float* p = I + ((size_t)c0[2] * ny + c0[1]) * nx + c0[0];
     const float a000 = __ldg(p), a100 = __ldg(p + dx);
     const float a010 = __ldg(p + dy), a110 = __ldg(p + dy + dx);
     const float a001 = __ldg(p + dz), a101 = __ldg(p + dz + dx);
     const float a011 = __ldg(p + dz + dy), a111 = __ldg(p + dz + dy + dx);
-    const float ux = 1.f - t[0], uy = 1.f - t[1], uz = 1.f - t[2];
-    const float c00 = fmaf(t[0], a100, ux * a000);
-    const float c10 = fmaf(t[0], a110, ux * a010);
-    const float c01 = fmaf(t[0], a101, ux * a001);
-    const float c11 = fmaf(t[0], a111, ux * a011);
-    const float e0 = fmaf(t[1], c10, uy * c00);
-    const float e1 = fmaf(t[1], c11, uy * c01);
-    return fmaf(t[2], e1, uz * e0);
+    const float c00 = fmaf(t[0], a100 - a000, a000);
+    const float c10 = fmaf(t[0], a110 - a010, a010);
+    const float c01 = fmaf(t[0], a101 - a001, a001);
+    const float c11 = fmaf(t[0], a111 - a011, a011);
+    const float e0 = fmaf(t[1], c10 - c00, c00);
+    const float e1 = fmaf(t[1], c11 - c01, c01);
+    return fmaf(t[2], e1 - e0, e0);
 }
 
 }  // namespace disc

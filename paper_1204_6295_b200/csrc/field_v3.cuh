@@ -27,48 +27,47 @@ struct TriSample {
     float tx, ty, tz;
 };
 
-// Cell and weight of one axis of the sample position p = clamp(i + r, 0, n - 1) (reading A11), WITHOUT forming i + r:
-// floor(i + r) = i + floor(r) and the weight r - floor(r) are exact in fp32, whereas fl(i + r) loses up to
-// ulp(i)/2 = 3e-5 voxel at i ~ 500 -- at a 1000 HU/voxel edge that is 0.03 HU of the warped image, the largest
-// single term of the whole-schedule field error before this change (profiles/r02_accuracy.md).
-// p < 0 -> cell 0, weight 0; p >= n - 1 -> cell n - 2, weight 1 (n >= 2).
-__device__ __forceinline__ void tri_axis(int i, float r, int n, int& i0, float& t) {
+// Cell, weight and neighbour direction of one axis of the sample position p = clamp(i + r, 0, n - 1) (reading A11),
+// WITHOUT forming i + r: floor(i + r) = i + floor(r) and the weight r - floor(r) are exact in fp32, whereas fl(i + r)
+// loses up to ulp(i)/2 = 3e-5 voxel at i ~ 500.  The lerp is a + t (b - a) with a = I[i0], b = I[i0 + step]:
+//   inside      i0 = i + floor(r), t = r - floor(r), step = +1
+//   p <= 0      i0 = 0,     t = 0, step = +1
+//   p >= n - 1  i0 = n - 1, t = 0, step = -1   (the neighbour is never out of the volume; n >= 2)
+// so a zero field, an integer shift and a clamped sample reproduce a voxel bit for bit (t = 0), and a flat region
+// stays flat bit for bit (b - a = 0): with (1 - t) a + t b a constant CT came out +-1 ulp noisy, which the patch
+// variance of step (a) turns into a spurious sigma_m and the demons force of a flat region amplifies.
+__device__ __forceinline__ void tri_axis(int i, float r, int n, int& i0, float& t, int& step) {
     const float fl = floorf(r);
     i0 = i + (int)fl;
     t = r - fl;
     const bool lo = i0 < 0, hi = i0 > n - 2;
-    i0 = lo ? 0 : (hi ? n - 2 : i0);
-    t = lo ? 0.f : (hi ? 1.f : t);
+    i0 = lo ? 0 : (hi ? n - 1 : i0);
+    t = (lo || hi) ? 0.f : t;
+    step = hi ? -1 : 1;
 }
 
-// FAST: every axis has at least two voxels (checked once per kernel, uniform), so the neighbour offsets are the
-// constants +1, +nx, +plane and the eight addresses share four row pointers.  (x, y, z): the voxel, (rx, ry, rz): its
-// displacement.
+// (x, y, z): the voxel, (rx, ry, rz): its displacement.  FAST: every axis has at least two voxels and the voxel
+// indices fit 32 bits (checked once per kernel, uniform).
 template <bool FAST>
 __device__ __forceinline__ void tri_issue(const float* __restrict__ I, int nx, int ny, int nz, int x, int y, int z,
                                           float rx, float ry, float rz, TriSample& s) {
+    int x0 = 0, y0 = 0, z0 = 0, sx = 0, sy = 0, sz = 0;
+    s.tx = 0.f; s.ty = 0.f; s.tz = 0.f;                // an axis of length 1 has weight 0 and no neighbour
+    if (FAST || nx > 1) tri_axis(x, rx, nx, x0, s.tx, sx);
+    if (FAST || ny > 1) tri_axis(y, ry, ny, y0, s.ty, sy);
+    if (FAST || nz > 1) tri_axis(z, rz, nz, z0, s.tz, sz);
     if (FAST) {
-        int x0, y0, z0;
-        tri_axis(x, rx, nx, x0, s.tx);
-        tri_axis(y, ry, ny, y0, s.ty);
-        tri_axis(z, rz, nz, z0, s.tz);
-        const float* p00 = I + ((size_t)(unsigned)((z0 * ny + y0) * nx + x0));
-        const float* p10 = p00 + nx;
-        const float* p01 = p00 + (size_t)nx * ny;
-        const float* p11 = p01 + nx;
-        s.a[0] = __ldg(p00); s.a[1] = __ldg(p00 + 1);
-        s.a[2] = __ldg(p10); s.a[3] = __ldg(p10 + 1);
-        s.a[4] = __ldg(p01); s.a[5] = __ldg(p01 + 1);
-        s.a[6] = __ldg(p11); s.a[7] = __ldg(p11 + 1);
+        const int dy = sy * nx, dz = sz * nx * ny;
+        const float* p00 = I + ((z0 * ny + y0) * nx + x0);
+        const float* p10 = p00 + dy;
+        const float* p01 = p00 + dz;
+        const float* p11 = p01 + dy;
+        s.a[0] = __ldg(p00); s.a[1] = __ldg(p00 + sx);
+        s.a[2] = __ldg(p10); s.a[3] = __ldg(p10 + sx);
+        s.a[4] = __ldg(p01); s.a[5] = __ldg(p01 + sx);
+        s.a[6] = __ldg(p11); s.a[7] = __ldg(p11 + sx);
     } else {
-        int x0 = 0, y0 = 0, z0 = 0;
-        s.tx = 0.f; s.ty = 0.f; s.tz = 0.f;            // an axis of length 1 has weight 0
-        if (nx > 1) tri_axis(x, rx, nx, x0, s.tx);
-        if (ny > 1) tri_axis(y, ry, ny, y0, s.ty);
-        if (nz > 1) tri_axis(z, rz, nz, z0, s.tz);
-        const int dx = nx > 1 ? 1 : 0;
-        const int dy = ny > 1 ? nx : 0;
-        const size_t dz = nz > 1 ? (size_t)nx * ny : 0;
+        const ptrdiff_t dx = sx, dy = (ptrdiff_t)sy * nx, dz = (ptrdiff_t)sz * nx * ny;
         const float* p = I + ((size_t)z0 * ny + y0) * nx + x0;
         s.a[0] = __ldg(p); s.a[1] = __ldg(p + dx);
         s.a[2] = __ldg(p + dy); s.a[3] = __ldg(p + dy + dx);
@@ -78,15 +77,14 @@ __device__ __forceinline__ void tri_issue(const float* __restrict__ I, int nx, i
 }
 
 __device__ __forceinline__ float tri_finish(const TriSample& s) {
-    // (1-t)*a + t*b: exact at t = 0 and t = 1, so a zero field reproduces the input bit for bit
-    const float ux = 1.f - s.tx, uy = 1.f - s.ty, uz = 1.f - s.tz;
-    const float c00 = fmaf(s.tx, s.a[1], ux * s.a[0]);
-    const float c10 = fmaf(s.tx, s.a[3], ux * s.a[2]);
-    const float c01 = fmaf(s.tx, s.a[5], ux * s.a[4]);
-    const float c11 = fmaf(s.tx, s.a[7], ux * s.a[6]);
-    const float c0 = fmaf(s.ty, c10, uy * c00);
-    const float c1 = fmaf(s.ty, c11, uy * c01);
-    return fmaf(s.tz, c1, uz * c0);
+    // a + t (b - a): exact at t = 0 and wherever the two neighbours are equal
+    const float c00 = fmaf(s.tx, s.a[1] - s.a[0], s.a[0]);
+    const float c10 = fmaf(s.tx, s.a[3] - s.a[2], s.a[2]);
+    const float c01 = fmaf(s.tx, s.a[5] - s.a[4], s.a[4]);
+    const float c11 = fmaf(s.tx, s.a[7] - s.a[6], s.a[6]);
+    const float c0 = fmaf(s.ty, c10 - c00, c00);
+    const float c1 = fmaf(s.ty, c11 - c01, c01);
+    return fmaf(s.tz, c1 - c0, c0);
 }
 
 // Step (b) alone (disc_warp) with two x-adjacent voxels per thread: 8-byte field loads and stores, both samples'

@@ -82,7 +82,7 @@ def test_moments3_anisotropic_ramp_closed_form(oracle_mod):
         np.testing.assert_allclose(mean[c], v[c], atol=1e-10)
 
 
-# ---------------------------------------------------------------- summed-area moments vs the naive loops
+# ---------------------------------------------------------------- exact (128-bit integer) summed-area moments vs the naive loops
 @pytest.mark.parametrize("shape", [(7, 6, 5), (4, 4, 4), (9, 1, 1), (1, 1, 9), (3, 8, 2)])
 @pytest.mark.parametrize("R", [0, 1, 2, 3, (3, 1, 2)])
 def test_sat_moments_match_naive(oracle_mod, shape, R):
@@ -98,15 +98,23 @@ def test_sat_moments_match_naive(oracle_mod, shape, R):
 
 
 def test_sat_moments_on_a_phantom(oracle_mod):
-    """HU-scale data with large flat regions (var = 0 exactly in the naive two-pass loop): the summed-area route stays
-    within 1e-6 HU^2 in variance, i.e. 1e-3 HU in sigma at worst, far inside the 1e-4 x range budget of the correction."""
+    """HU-scale data with large flat regions: the summed-area route is exact integer arithmetic up to the one final
+    conversion, so a flat patch has var = 0 EXACTLY (as in the naive two-pass loop) and everywhere else the two agree
+    to the naive loop's own fp64 rounding.  (With fp64 tables the error was 1e-6 HU^2, i.e. a spurious sigma of
+    1e-3 HU in flat air, enough to move the whole-schedule field of config 4 by 1e-2 voxel.)"""
     ct, cbct, _, _ = phantoms.make_pair(1, dims=(40, 36, 20))
     for v, R in ((ct, 3), (cbct, (4, 4, 1))):
         mean, var = oracle_mod.box_moments3(v, R)
         ms, vs = oracle_mod.box_moments3(v, R, sat=True)
-        assert np.abs(ms - mean).max() < 1e-9
-        assert np.abs(vs - var).max() < 1e-6
+        assert np.abs(ms - mean).max() < 1e-11
+        assert np.abs(vs - var).max() < 1e-8 and (np.abs(vs - var) <= 1e-12 * var + 1e-13).all()
         assert vs.min() >= 0.0
+        assert ((var == 0.0) == (vs == 0.0)).all() and (var == 0.0).any() == (v is ct)
+    # values below 2^-7 HU are rounded to 2^-30 HU; values beyond +-16384 are refused (outputs left untouched)
+    tiny = np.array([[[1e-3, 2e-3, -3e-3, 5e-4]]], dtype=np.float32)
+    m1, v1 = oracle_mod.box_moments3(tiny, (1, 0, 0))
+    m2, v2 = oracle_mod.box_moments3(tiny, (1, 0, 0), sat=True)
+    assert np.abs(m1 - m2).max() < 1e-9 and np.abs(v1 - v2).max() < 1e-11
 
 
 # ---------------------------------------------------------------- NEXT-4: pyramid with per-axis factors
