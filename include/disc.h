@@ -36,7 +36,7 @@ typedef struct disc_ctx disc_ctx; /* opaque, owned by the library */
 typedef enum {
     DISC_OK = 0,
     DISC_ERR_INVALID_ARG = 1,
-    DISC_ERR_UNSUPPORTED = 2, /* no sm_100 device, patch_radius > 10, Gaussian radius > 12 */
+    DISC_ERR_UNSUPPORTED = 2, /* no sm_100 device, patch radius > 12 or Rx != Ry, Gaussian radius > 12 */
     DISC_ERR_ALLOC = 3,
     DISC_ERR_CUDA = 4
 } disc_status;
@@ -67,6 +67,25 @@ typedef enum {
  */
 disc_status disc_create(disc_ctx** out, const int dims[3], const float spacing[3], int patch_radius,
                         float sigma_smooth, int levels, int iters);
+
+/*
+ * disc_create_ex -- the same with the clinical geometry of the paper: a non-cubic patch and a pyramid
+ * that need not halve every axis.
+ *   patch_radius    (Rx, Ry, Rz) >= 0, HOST: the patch is the box of side 2R_c + 1 along axis c.  The paper's patches are
+ *                   3x3x3 ... 25x25x7, i.e. radii up to (12, 12, 3); all have Rx == Ry, and that is
+ *                   what this build supports: Rx != Ry, or a radius > DISC_MAX_PATCH_RADIUS -> DISC_ERR_UNSUPPORTED.
+ *   pyramid_factor  (fx, fy, fz), each 1 or 2, HOST: level l has dims[c] / f_c^l voxels along axis c (each must divide).
+ *                   The paper's clinical volumes (256x256x68 at 0.94x0.94x2.5 mm) were down-sampled in the transverse
+ *                   plane only: factor (2, 2, 1).  Down: block mean over fx*fy*fz voxels; up: trilinear at
+ *                   i/2 - 1/4 along the halved axes, identity along the others; component c of the field is scaled by
+ *                   f_c, because it is in voxel units of its own axis (reading A9).
+ *   spacing         recorded, never used by the iteration: Eq. (1) has no spacing term and the paper runs
+ *                   its anisotropic volumes with the same formula, so gradients are per voxel, the Gaussian sigma is in
+ *                   voxels on every axis and the field is in voxels of its own axis (reading A13).
+ * Everything else as disc_create, which is disc_create_ex with (R, R, R) and (2, 2, 2).
+ */
+disc_status disc_create_ex(disc_ctx** out, const int dims[3], const float spacing[3], const int patch_radius[3],
+                           float sigma_smooth, int levels, int iters, const int pyramid_factor[3]);
 
 /* Synchronises the device, frees the context and its scratch.  NULL is allowed. */
 void disc_destroy(disc_ctx* ctx);
@@ -166,12 +185,12 @@ disc_status disc_force_update(disc_ctx* ctx, int level, const float* m, const fl
 /* Step (d) alone: disp_inout <- G_sigma * disp_inout. */
 disc_status disc_smooth_field(disc_ctx* ctx, int level, float* disp_inout, void* stream);
 
-/* 2x2x2 block mean from level_from to level_from+1 (reading A9).
- * vol [N_level_from], out [N_level_from / 8]. */
+/* Block mean from level_from to level_from+1 over the context's pyramid factor, 2x2x2 by default (
+ * reading A9).  vol [N_level_from], out [N_level_from+1]. */
 disc_status disc_downsample(disc_ctx* ctx, int level_from, const float* vol, float* out, void* stream);
 
-/* x2 trilinear up-sampling of a field from level_from to level_from-1 at i/2 - 1/4 (clamped), values
- * doubled (reading A9).  disp [3*N_level_from], out [3*8*N_level_from]. */
+/* Up-sampling of a field from level_from to level_from-1: trilinear at i/2 - 1/4 (clamped) with the value doubled
+ * along every axis the pyramid halves (reading A9).  disp [3*N_level_from], out [3*N_level_from-1]. */
 disc_status disc_upsample_field(disc_ctx* ctx, int level_from, const float* disp, float* out, void* stream);
 
 #ifdef __cplusplus

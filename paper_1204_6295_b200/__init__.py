@@ -16,14 +16,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdisc.so")
 
 DISC_OK, DISC_ERR_INVALID_ARG, DISC_ERR_UNSUPPORTED, DISC_ERR_ALLOC, DISC_ERR_CUDA = range(5)
-DISC_MAX_PATCH_RADIUS = 10
+DISC_MAX_PATCH_RADIUS = 12
 DISC_MAX_GAUSS_RADIUS = 12
 DISC_EPS_VAR = 1e-6
 DISC_EPS_DEN = 1e-3
 DISC_FORCE_THIRION, DISC_FORCE_DOUBLE = 1, 2
 
 EXPORTS = (
-    "disc_create", "disc_destroy", "disc_last_error", "disc_launch_count", "disc_set_force", "disc_set_stop", "disc_iterations_run", "disc_warp", "disc_correct_intensity",
+    "disc_create", "disc_create_ex", "disc_destroy", "disc_last_error", "disc_launch_count", "disc_set_force", "disc_set_stop", "disc_iterations_run", "disc_warp", "disc_correct_intensity",
     "disc_demons_step", "disc_register", "disc_register_host", "disc_iterate", "disc_box_moments",
     "disc_force_update", "disc_smooth_field", "disc_downsample", "disc_upsample_field", "disc_profile_iteration",
 )
@@ -38,6 +38,9 @@ _vp, _i = ctypes.c_void_p, ctypes.c_int
 _lib.disc_create.restype = _i
 _lib.disc_create.argtypes = [ctypes.POINTER(_vp), ctypes.POINTER(_i), ctypes.POINTER(ctypes.c_float), _i,
                              ctypes.c_float, _i, _i]
+_lib.disc_create_ex.restype = _i
+_lib.disc_create_ex.argtypes = [ctypes.POINTER(_vp), ctypes.POINTER(_i), ctypes.POINTER(ctypes.c_float), ctypes.POINTER(_i),
+                                ctypes.c_float, _i, _i, ctypes.POINTER(_i)]
 _lib.disc_destroy.restype = None
 _lib.disc_destroy.argtypes = [_vp]
 _lib.disc_last_error.restype = ctypes.c_char_p
@@ -94,17 +97,23 @@ def _x3(n):
     return None if n is None else 3 * n
 
 
-def _host(a):
-    """host pointer of a float32 C-contiguous numpy array or CPU tensor (None -> NULL)"""
+def _host(a, numel=None):
+    """host pointer of a float32 C-contiguous numpy array or CPU tensor with `numel` elements (None -> NULL)"""
     if a is None:
         return None
     if hasattr(a, "data_ptr"):
-        if a.is_cuda or not a.is_contiguous() or a.element_size() != 4:
+        import torch
+        if a.is_cuda or not a.is_contiguous() or a.dtype != torch.float32:
             raise TypeError("expected a contiguous float32 CPU tensor")
-        return a.data_ptr()
-    if a.dtype.itemsize != 4 or not a.flags["C_CONTIGUOUS"]:
-        raise TypeError("expected a C-contiguous float32 numpy array")
-    return a.ctypes.data
+        n, ptr = a.numel(), a.data_ptr()
+    else:
+        import numpy as np
+        if a.dtype != np.float32 or not a.flags["C_CONTIGUOUS"]:
+            raise TypeError("expected a C-contiguous float32 numpy array")
+        n, ptr = a.size, a.ctypes.data
+    if numel is not None and n != int(numel):
+        raise ValueError(f"host buffer has {n} elements, expected {numel}")
+    return ptr
 
 
 def _stream(stream):
@@ -117,17 +126,22 @@ def _stream(stream):
 class Ctx:
     """Opaque handle returned by disc_create (keeps the level sizes for argument checks)."""
 
-    def __init__(self, handle, dims, levels):
+    def __init__(self, handle, dims, levels, pyramid_factor=(2, 2, 2)):
         self.handle = handle
         self.dims = tuple(dims)
         self.levels = levels
+        self.pyramid_factor = tuple(pyramid_factor)
+
+    def level_dims(self, level):
+        """(nx, ny, nz) at `level`"""
+        return tuple(d // f ** level for d, f in zip(self.dims, self.pyramid_factor))
 
     def n(self, level):
         """voxels at `level`; None for a level the context does not have (the C layer reports that)"""
         if not 0 <= level < self.levels:
             return None
-        nx, ny, nz = self.dims
-        return (nx >> level) * (ny >> level) * (nz >> level)
+        nx, ny, nz = self.level_dims(level)
+        return nx * ny * nz
 
     def __del__(self):
         h, self.handle = getattr(self, "handle", None), None
@@ -142,6 +156,18 @@ def disc_create(dims, spacing, patch_radius, sigma_smooth, levels, iters) -> Ctx
     st = _lib.disc_create(ctypes.byref(out), d, s, int(patch_radius), float(sigma_smooth), int(levels), int(iters))
     _check(None, st)
     return Ctx(out.value, dims, levels)
+
+
+def disc_create_ex(dims, spacing, patch_radius, sigma_smooth, levels, iters, pyramid_factor=(2, 2, 2)) -> Ctx:
+    """patch_radius = (Rx, Ry, Rz), pyramid_factor = (fx, fy, fz) with each factor 1 or 2"""
+    out = _vp()
+    d = (_i * 3)(*[int(v) for v in dims])
+    s = (ctypes.c_float * 3)(*[float(v) for v in spacing])
+    r = (_i * 3)(*[int(v) for v in patch_radius])
+    f = (_i * 3)(*[int(v) for v in pyramid_factor])
+    st = _lib.disc_create_ex(ctypes.byref(out), d, s, r, float(sigma_smooth), int(levels), int(iters), f)
+    _check(None, st)
+    return Ctx(out.value, dims, levels, pyramid_factor)
 
 
 def disc_destroy(ctx: Ctx) -> None:
@@ -198,8 +224,9 @@ def disc_register(ctx, ct, cbct, out_disp, out_corrected_cbct, stream=None):
 
 
 def disc_register_host(ctx, ct_host, cbct_host, out_disp_host, out_corrected_cbct_host, stream=None):
-    _check(ctx.handle, _lib.disc_register_host(ctx.handle, _host(ct_host), _host(cbct_host), _host(out_disp_host),
-                                               _host(out_corrected_cbct_host), _stream(stream)))
+    n = ctx.n(0)
+    _check(ctx.handle, _lib.disc_register_host(ctx.handle, _host(ct_host, n), _host(cbct_host, n), _host(out_disp_host, 3 * n),
+                                               _host(out_corrected_cbct_host, n), _stream(stream)))
 
 
 def disc_iterate(ctx, level, ct, cbct, disp_inout, n_iters, stream=None):

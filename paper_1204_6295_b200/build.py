@@ -20,7 +20,7 @@ LIB = os.path.join(HERE, "libdisc.so")
 # no --use_fast_math: IEEE division and sqrt are kept
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 
-R_RANGES = [(0, 3), (4, 5), (6, 7), (8, 10)]
+R_RANGES = [(0, 3), (4, 6), (7, 9), (10, 12)]
 K_RANGES = [(1, 3), (4, 6), (7, 9), (10, 12)]
 
 def _units():

@@ -35,7 +35,8 @@ thread_local char g_create_error[256] = "";
 struct disc_ctx {
     int dims[3];
     float spacing[3];
-    int R;
+    int R[3];         // patch radius per axis (R[0] == R[1])
+    int fac[3];       // pyramid factor per axis, 1 or 2
     float sigma;
     int levels, iters;
     int K;
@@ -98,8 +99,8 @@ disc_status check_device(disc_ctx* c) {
 template <int MODE>
 disc_status launch_moments(disc_ctx* c, const Level& L, const float* vol, const float* aux, float* out0,
                            float* out1, IterCtl ctl, cudaStream_t st) {
-    if (!launch_moments_any(c->di, c->R, c->R, MODE, vol, aux, out0, out1, L.nx, L.ny, L.nz, DISC_EPS_VAR, ctl, st))
-        return fail(c, DISC_ERR_UNSUPPORTED, "no moments kernel for patch radius %d on %dx%dx%d", c->R, L.nx, L.ny, L.nz);
+    if (!launch_moments_any(c->di, c->R[0], c->R[2], MODE, vol, aux, out0, out1, L.nx, L.ny, L.nz, DISC_EPS_VAR, ctl, st))
+        return fail(c, DISC_ERR_UNSUPPORTED, "no moments kernel for patch radius (%d,%d,%d)", c->R[0], c->R[1], c->R[2]);
     return check_launch(c, "k_moments");
 }
 
@@ -126,16 +127,22 @@ disc_status launch_warp(disc_ctx* c, const Level& L, const float* moving, const 
 }
 
 disc_status launch_downsample(disc_ctx* c, const Level& fine, const float* in, float* out, cudaStream_t st) {
-    const int mx = fine.nx / 2, my = fine.ny / 2, mz = fine.nz / 2;
+    const int* f = c->fac;
+    const int mx = fine.nx / f[0], my = fine.ny / f[1], mz = fine.nz / f[2];
     dim3 grid((mx + 127) / 128, my, mz);
-    k_downsample<<<grid, 128, 0, st>>>(in, out, mx, my, mz);
+    // 8-byte loads of the two x neighbours need an even row length (it is: nx = 2 mx) and an 8-byte aligned base
+    if (f[0] == 2 && (reinterpret_cast<uintptr_t>(in) & 7u) == 0)
+        k_downsample<true><<<grid, 128, 0, st>>>(in, out, mx, my, mz, f[0], f[1], f[2]);
+    else
+        k_downsample<false><<<grid, 128, 0, st>>>(in, out, mx, my, mz, f[0], f[1], f[2]);
     return check_launch(c, "k_downsample");
 }
 
 disc_status launch_upsample(disc_ctx* c, const Level& coarse, const float* in, float* out, cudaStream_t st) {
-    const int nx = 2 * coarse.nx, ny = 2 * coarse.ny, nz = 2 * coarse.nz;
+    const int* f = c->fac;
+    const int nx = f[0] * coarse.nx, ny = f[1] * coarse.ny, nz = f[2] * coarse.nz;
     dim3 grid((nx + 127) / 128, ny, 3 * nz);
-    k_upsample_field<<<grid, 128, 0, st>>>(in, out, coarse.nx, coarse.ny, coarse.nz);
+    k_upsample_field<<<grid, 128, 0, st>>>(in, out, coarse.nx, coarse.ny, coarse.nz, f[0], f[1], f[2]);
     return check_launch(c, "k_upsample_field");
 }
 
@@ -188,21 +195,33 @@ extern "C" {
 
 disc_status disc_create(disc_ctx** out, const int dims[3], const float spacing[3], int patch_radius,
                         float sigma_smooth, int levels, int iters) {
+    const int R3[3] = {patch_radius, patch_radius, patch_radius}, f3[3] = {2, 2, 2};
+    return disc_create_ex(out, dims, spacing, R3, sigma_smooth, levels, iters, f3);
+}
+
+disc_status disc_create_ex(disc_ctx** out, const int dims[3], const float spacing[3], const int patch_radius[3],
+                           float sigma_smooth, int levels, int iters, const int pyramid_factor[3]) {
     if (!out) return fail(nullptr, DISC_ERR_INVALID_ARG, "out is NULL");
     *out = nullptr;
-    if (!dims || !spacing) return fail(nullptr, DISC_ERR_INVALID_ARG, "dims/spacing is NULL");
+    if (!dims || !spacing || !patch_radius || !pyramid_factor)
+        return fail(nullptr, DISC_ERR_INVALID_ARG, "dims/spacing/patch_radius/pyramid_factor is NULL");
     if (levels < 1 || levels > DISC_MAX_LEVELS) return fail(nullptr, DISC_ERR_INVALID_ARG, "levels must be in 1..%d", DISC_MAX_LEVELS);
     for (int i = 0; i < 3; ++i) {
         if (dims[i] < 1) return fail(nullptr, DISC_ERR_INVALID_ARG, "dims[%d] < 1", i);
         if (!(spacing[i] > 0.f)) return fail(nullptr, DISC_ERR_INVALID_ARG, "spacing[%d] <= 0", i);
-        if (dims[i] % (1 << (levels - 1)) != 0)
+        if (pyramid_factor[i] != 1 && pyramid_factor[i] != 2)
+            return fail(nullptr, DISC_ERR_INVALID_ARG, "pyramid_factor[%d] must be 1 or 2", i);
+        if (pyramid_factor[i] == 2 && dims[i] % (1 << (levels - 1)) != 0)
             return fail(nullptr, DISC_ERR_INVALID_ARG, "dims[%d]=%d not divisible by 2^(levels-1)", i, dims[i]);
+        if (patch_radius[i] < 0) return fail(nullptr, DISC_ERR_INVALID_ARG, "patch_radius < 0");
     }
-    if (patch_radius < 0) return fail(nullptr, DISC_ERR_INVALID_ARG, "patch_radius < 0");
     if (!(sigma_smooth > 0.f)) return fail(nullptr, DISC_ERR_INVALID_ARG, "sigma_smooth <= 0");
     if (iters < 0) return fail(nullptr, DISC_ERR_INVALID_ARG, "iters < 0");
-    if (patch_radius > DISC_MAX_PATCH_RADIUS)
-        return fail(nullptr, DISC_ERR_UNSUPPORTED, "patch_radius %d > %d", patch_radius, DISC_MAX_PATCH_RADIUS);
+    for (int i = 0; i < 3; ++i)
+        if (patch_radius[i] > DISC_MAX_PATCH_RADIUS)
+            return fail(nullptr, DISC_ERR_UNSUPPORTED, "patch_radius %d > %d", patch_radius[i], DISC_MAX_PATCH_RADIUS);
+    if (patch_radius[0] != patch_radius[1])
+        return fail(nullptr, DISC_ERR_UNSUPPORTED, "patch radii along x and y must be equal (%d != %d)", patch_radius[0], patch_radius[1]);
     const int K = (int)std::ceil(3.0 * (double)sigma_smooth);
     if (K > DISC_MAX_GAUSS_RADIUS)
         return fail(nullptr, DISC_ERR_UNSUPPORTED, "Gaussian radius ceil(3 sigma) = %d > %d", K, DISC_MAX_GAUSS_RADIUS);
@@ -223,7 +242,8 @@ disc_status disc_create(disc_ctx** out, const int dims[3], const float spacing[3
     c->di.dev = dev;
     c->di.n_sm = 148;
     cudaDeviceGetAttribute(&c->di.n_sm, cudaDevAttrMultiProcessorCount, dev);
-    c->R = patch_radius; c->sigma = sigma_smooth; c->levels = levels; c->iters = iters; c->K = K;
+    for (int i = 0; i < 3; ++i) { c->R[i] = patch_radius[i]; c->fac[i] = pyramid_factor[i]; }
+    c->sigma = sigma_smooth; c->levels = levels; c->iters = iters; c->K = K;
     c->force_mode = DISC_FORCE_THIRION;
     c->stop_eps = -1.f;
     if (cudaMalloc(&c->d_stop, sizeof(StopCtl)) != cudaSuccess || cudaMemset(c->d_stop, 0, sizeof(StopCtl)) != cudaSuccess) {
@@ -239,7 +259,8 @@ disc_status disc_create(disc_ctx** out, const int dims[3], const float spacing[3
     }
     for (int l = 0; l < levels; ++l) {
         Level& L = c->lv[l];
-        L.nx = dims[0] >> l; L.ny = dims[1] >> l; L.nz = dims[2] >> l;
+        L.nx = dims[0]; L.ny = dims[1]; L.nz = dims[2];
+        for (int i = 0; i < l; ++i) { L.nx /= c->fac[0]; L.ny /= c->fac[1]; L.nz /= c->fac[2]; }
         L.N = (size_t)L.nx * L.ny * L.nz;
         const size_t b = L.N * sizeof(float);
         bool ok = cudaMalloc(&L.zhat, b) == cudaSuccess && cudaMalloc(&L.m, b) == cudaSuccess &&

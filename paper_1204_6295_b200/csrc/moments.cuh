@@ -180,4 +180,45 @@ k_moments(const float* __restrict__ vol, const float* __restrict__ aux, float* _
     }
 }
 
+// The plain definition, one thread per voxel looping over its whole patch (as the paper's own kernel does,
+// PAPER.md:410), for what the sliding-window kernels do not cover: a non-cubic patch
+// on a volume the TMA kernel cannot take (nx % 4 != 0, unaligned base) or with a z radius beyond its tensor-memory
+// ring.  fp64 sums over the truncated box (reading A4), cost proportional to the patch: a fallback, not a fast path.
+template <int MODE>
+__global__ void __launch_bounds__(128)
+k_moments_direct(const float* __restrict__ vol, const float* __restrict__ aux, float* __restrict__ out0,
+                 float* __restrict__ out1, int nx, int ny, int nz, int rx, int ry, int rz, float eps_var, IterCtl ctl) {
+    if (iter_skipped(ctl)) return;
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y, z = blockIdx.z;
+    if (x >= nx) return;
+    const int xa = max(x - rx, 0), xb = min(x + rx, nx - 1);
+    const int ya = max(y - ry, 0), yb = min(y + ry, ny - 1);
+    const int za = max(z - rz, 0), zb = min(z + rz, nz - 1);
+    double s1 = 0.0, s2 = 0.0;
+    for (int c = za; c <= zb; ++c)
+        for (int b = ya; b <= yb; ++b) {
+            const float* row = vol + ((size_t)c * ny + b) * nx;
+            for (int a = xa; a <= xb; ++a) {
+                const double v = (double)__ldg(row + a);
+                s1 += v;
+                s2 = fma(v, v, s2);
+            }
+        }
+    const double inv_n = 1.0 / ((double)(xb - xa + 1) * (double)(yb - ya + 1) * (double)(zb - za + 1));
+    const double mu = s1 * inv_n;
+    const double var = fmax(fma(-mu, mu, s2 * inv_n), 0.0);
+    const size_t idx = ((size_t)z * ny + y) * nx + x;
+    if (MODE == kModeMoments) {
+        out0[idx] = (float)mu;
+        out1[idx] = (float)var;
+    } else if (MODE == kModeZscore) {
+        const float varf = (float)var;
+        const float dv = (float)((double)__ldg(vol + idx) - mu);
+        out0[idx] = var > (double)eps_var ? dv * rsqrtf(varf) : 0.f;
+    } else {
+        out0[idx] = fmaf(sqrtf((float)var), __ldg(aux + idx), (float)mu);
+    }
+}
+
 }  // namespace disc

@@ -26,6 +26,18 @@ static EncodeTiledFn encode_tiled() {
     return fn;
 }
 
+// the plain definition for everything the sliding-window kernels do not cover (moments.cuh)
+static void launch_moments_direct(int rx, int ry, int rz, int mode, const float* vol, const float* aux, float* out0,
+                                  float* out1, int nx, int ny, int nz, float eps_var, IterCtl ctl, cudaStream_t st) {
+    dim3 grid((nx + 127) / 128, ny, nz);
+    if (mode == kModeMoments)
+        k_moments_direct<kModeMoments><<<grid, 128, 0, st>>>(vol, aux, out0, out1, nx, ny, nz, rx, ry, rz, eps_var, ctl);
+    else if (mode == kModeZscore)
+        k_moments_direct<kModeZscore><<<grid, 128, 0, st>>>(vol, aux, out0, out1, nx, ny, nz, rx, ry, rz, eps_var, ctl);
+    else
+        k_moments_direct<kModeCorrect><<<grid, 128, 0, st>>>(vol, aux, out0, out1, nx, ny, nz, rx, ry, rz, eps_var, ctl);
+}
+
 // z chunk of the marching kernels: minimise (waves of CTAs) x (slices marched per CTA, with the 2 rz halo and a few
 // slices of pipeline fill).  `slots` = CTAs resident on the device at once.
 static int pick_zchunk(long long tiles, long long slots, int nz, int rz) {
@@ -102,7 +114,7 @@ static bool launch_r(const DevInfo& di, int rz, int mode, const float* vol, cons
         launch_r_tma<R>(di, rz, mode, vol, aux, out0, out1, nx, ny, nz, eps_var, ctl, st))
         return true;
     if constexpr (R <= 10) {
-        if (rz == R) {   // plain-load kernel: cubic patches, any nx
+        if (rz == R) {   // plain-load sliding-window kernel: cubic patches, any nx
             const long long tiles = (long long)((nx + kMomTX - 1) / kMomTX) * ((ny + kMomTY - 1) / kMomTY);
             const int zchunk = pick_zchunk(tiles, 2LL * di.n_sm, nz, rz);
             dim3 grid((nx + kMomTX - 1) / kMomTX, (ny + kMomTY - 1) / kMomTY, (nz + zchunk - 1) / zchunk);
@@ -116,7 +128,8 @@ static bool launch_r(const DevInfo& di, int rz, int mode, const float* vol, cons
             return true;
         }
     }
-    return false;
+    launch_moments_direct(R, R, rz, mode, vol, aux, out0, out1, nx, ny, nz, eps_var, ctl, st);
+    return true;
 }
 
 // one radius: launches if R lies in this unit's range (the discarded branch is never instantiated)

@@ -290,7 +290,8 @@ k_moments_v3(const __grid_constant__ CUtensorMap tmap, const float* __restrict__
                         r0 = (float)mu;
                     } else if (MODE == kModeZscore) {
                         const float dv = (float)((double)pre[o] - mu);
-                        r0 = varf > eps_var ? dv * rsqrt_nr(varf) : 0.f;
+                        // reading A5: the threshold decision is taken on the fp64 variance
+                        r0 = nvar * inv_n > (double)eps_var ? dv * rsqrt_nr(varf) : 0.f;
                     } else {
                         // branch free: 0 * rsqrt(tiny) = 0 where the variance is zero
                         const float sd = varf * rsqrt_nr(fmaxf(varf, 1e-30f));

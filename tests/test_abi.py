@@ -55,7 +55,7 @@ def test_create_validates_arguments_before_touching_the_device(lib):
         with pytest.raises(lib.DiscError) as e:
             lib.disc_create(**args)
         assert e.value.status == lib.DISC_ERR_INVALID_ARG, kw
-    for kw in (dict(patch_radius=11), dict(sigma_smooth=4.5)):
+    for kw in (dict(patch_radius=13), dict(sigma_smooth=4.5)):
         args = dict(dims=(8, 8, 8), spacing=(1, 1, 1), patch_radius=1, sigma_smooth=1.0, levels=1, iters=1)
         args.update(kw)
         with pytest.raises(lib.DiscError) as e:
