@@ -121,6 +121,47 @@ disc_status disc_set_force(disc_ctx* ctx, int mode);
  * return at once, so there is no host synchronisation.  Host-side state only, no launch. */
 disc_status disc_set_stop(disc_ctx* ctx, float eps);
 
+/*
+ * Reliability mask and interpolation / extrapolation of a, b (Alg. A1 step 2).
+ * With enable != 0, disc_register, disc_iterate and disc_correct_intensity replace the direct correction by
+ *   a = STD(M)/STD(S), b = E(M) - a E(S)                                   Eqs. (5)-(6)
+ *   xi = 1 where |I_m^(k) - I_s| > HU_0 or a < a_min or a > a_max          Eq. (7),
+ *   a = b = 0 where xi = 1, then, repeated until nothing is left: every voxel with xi = 1 takes the average of the
+ *   a, b of the available voxels (xi = 0, or filled by an earlier pass) in the cube T of radius fill_radius around
+ *   it, weighted by w_i = exp(-(I_s(i) - I_s(x))^2 / h^2)                  Eqs. (8)-(10)
+ *   I'_s = a I_s + b
+ * and disc_register first shifts the CBCT by Delta HU = mean(CT) - mean(CBCT) (Alg. A1 "globally adjust").
+ *   hu0             HU_0 [HU]; < 0: 2 |Delta HU|
+ *   a_min, a_max    bounds of a; a_min < 0: 0.5 a_m and 1.5 a_m with a_m the median of A computed before the DIR from the
+ *                   full-resolution images.  Reading A17: the median runs over the voxels where both patch
+ *                   variances exceed DISC_EPS_VAR and is the lower median.
+ *   fill_radius     radius of T in voxels, 1..8 (its size is lost from the text: "a relative small size")
+ *   h               Eq. (10) [HU], > 0 (never given in the text)
+ *   max_fill_passes 1..254; readings A18: a pass reads only what was available when it started; the weights are
+ *                   normalised by the largest one (same quotient, no underflow); passes stop when nothing is left, when a
+ *                   pass fills nothing or after max_fill_passes, and what is then still unfilled keeps a = b = 0.
+ * Everything is decided on the device (parameters, "anything left"): the iteration gets no host synchronisation.
+ * disc_set_mask itself allocates 4 N floats + N bytes per level on first use and copies the given parameters to the
+ * device (a blocking cudaMemcpy of a few bytes); until disc_mask_params or disc_register has derived them, a parameter
+ * given as < 0 reads HU_0 = 0, a_min = 0.5, a_max = 1.5.  enable == 0 switches back.
+ */
+disc_status disc_set_mask(disc_ctx* ctx, int enable, float hu0, float a_min, float a_max, int fill_radius, float h,
+                          int max_fill_passes);
+
+/* The parameters the mask derives from the two full-resolution images (device pointers), computed now and kept for
+ * later fine-grained calls: out_host = {Delta HU, HU_0, a_m, a_min, a_max} (HOST, 5 floats).  SYNCHRONISES `stream`. */
+disc_status disc_mask_params(disc_ctx* ctx, const float* ct, const float* cbct, float out_host[5], void* stream);
+
+/* a(x), b(x) and the mask of `level` as the last correction left them (device buffers, each may be NULL): out_a, out_b
+ * [N_level] floats, out_xi [N_level] bytes -- 0: xi = 0, k in 1..254: xi = 1, filled in pass k, 255: xi = 1, never filled. */
+disc_status disc_get_ab(disc_ctx* ctx, int level, float* out_a, float* out_b, unsigned char* out_xi, void* stream);
+
+/* Fig. 9 (e), (f) of the paper: the averages of a and of b over all voxels in every iteration of
+ * disc_register.  disc_get_diagnostics SYNCHRONISES the device and writes levels*iters doubles each (HOST), level-major
+ * from the COARSEST level, `iters` slots per level.  Without the mask this costs one more moments launch per iteration. */
+disc_status disc_set_diagnostics(disc_ctx* ctx, int enable);
+disc_status disc_get_diagnostics(disc_ctx* ctx, double* mean_a_host, double* mean_b_host);
+
 /* Iterations actually run per level by the last disc_register / disc_iterate on this context:
  * out_host[level], level = 0 .. levels-1 (HOST array of `levels` ints).  SYNCHRONISES the device when the
  * stopping criterion is enabled; without it the counts are the requested ones. */

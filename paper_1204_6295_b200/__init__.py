@@ -23,7 +23,7 @@ DISC_EPS_DEN = 1e-3
 DISC_FORCE_THIRION, DISC_FORCE_DOUBLE = 1, 2
 
 EXPORTS = (
-    "disc_create", "disc_create_ex", "disc_destroy", "disc_last_error", "disc_launch_count", "disc_set_force", "disc_set_stop", "disc_iterations_run", "disc_warp", "disc_correct_intensity",
+    "disc_create", "disc_create_ex", "disc_destroy", "disc_last_error", "disc_launch_count", "disc_set_force", "disc_set_stop", "disc_iterations_run", "disc_set_mask", "disc_mask_params", "disc_get_ab", "disc_set_diagnostics", "disc_get_diagnostics", "disc_warp", "disc_correct_intensity",
     "disc_demons_step", "disc_register", "disc_register_host", "disc_iterate", "disc_box_moments",
     "disc_force_update", "disc_smooth_field", "disc_downsample", "disc_upsample_field", "disc_profile_iteration",
 )
@@ -53,6 +53,16 @@ _lib.disc_set_stop.restype = _i
 _lib.disc_set_stop.argtypes = [_vp, ctypes.c_float]
 _lib.disc_iterations_run.restype = _i
 _lib.disc_iterations_run.argtypes = [_vp, ctypes.POINTER(_i)]
+_lib.disc_set_mask.restype = _i
+_lib.disc_set_mask.argtypes = [_vp, _i, ctypes.c_float, ctypes.c_float, ctypes.c_float, _i, ctypes.c_float, _i]
+_lib.disc_mask_params.restype = _i
+_lib.disc_mask_params.argtypes = [_vp, _vp, _vp, ctypes.POINTER(ctypes.c_float), _vp]
+_lib.disc_get_ab.restype = _i
+_lib.disc_get_ab.argtypes = [_vp, _i, _vp, _vp, _vp, _vp]
+_lib.disc_set_diagnostics.restype = _i
+_lib.disc_set_diagnostics.argtypes = [_vp, _i]
+_lib.disc_get_diagnostics.restype = _i
+_lib.disc_get_diagnostics.argtypes = [_vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
 for _name, _nptr in (("disc_warp", 3), ("disc_correct_intensity", 3), ("disc_demons_step", 3),
                      ("disc_box_moments", 3), ("disc_force_update", 3), ("disc_smooth_field", 1),
                      ("disc_downsample", 2), ("disc_upsample_field", 2)):
@@ -126,8 +136,9 @@ def _stream(stream):
 class Ctx:
     """Opaque handle returned by disc_create (keeps the level sizes for argument checks)."""
 
-    def __init__(self, handle, dims, levels, pyramid_factor=(2, 2, 2)):
+    def __init__(self, handle, dims, levels, pyramid_factor=(2, 2, 2), iters=0):
         self.handle = handle
+        self.iters = int(iters)
         self.dims = tuple(dims)
         self.levels = levels
         self.pyramid_factor = tuple(pyramid_factor)
@@ -155,7 +166,7 @@ def disc_create(dims, spacing, patch_radius, sigma_smooth, levels, iters) -> Ctx
     s = (ctypes.c_float * 3)(*[float(v) for v in spacing])
     st = _lib.disc_create(ctypes.byref(out), d, s, int(patch_radius), float(sigma_smooth), int(levels), int(iters))
     _check(None, st)
-    return Ctx(out.value, dims, levels)
+    return Ctx(out.value, dims, levels, iters=iters)
 
 
 def disc_create_ex(dims, spacing, patch_radius, sigma_smooth, levels, iters, pyramid_factor=(2, 2, 2)) -> Ctx:
@@ -167,7 +178,7 @@ def disc_create_ex(dims, spacing, patch_radius, sigma_smooth, levels, iters, pyr
     f = (_i * 3)(*[int(v) for v in pyramid_factor])
     st = _lib.disc_create_ex(ctypes.byref(out), d, s, r, float(sigma_smooth), int(levels), int(iters), f)
     _check(None, st)
-    return Ctx(out.value, dims, levels, pyramid_factor)
+    return Ctx(out.value, dims, levels, pyramid_factor, iters)
 
 
 def disc_destroy(ctx: Ctx) -> None:
@@ -191,6 +202,42 @@ def disc_set_force(ctx, mode):
 
 def disc_set_stop(ctx, eps):
     _check(ctx.handle, _lib.disc_set_stop(ctx.handle, float(eps)))
+
+
+def disc_set_mask(ctx, enable, hu0=-1.0, a_min=-1.0, a_max=-1.0, fill_radius=1, h=50.0, max_fill_passes=64):
+    _check(ctx.handle, _lib.disc_set_mask(ctx.handle, int(bool(enable)), float(hu0), float(a_min), float(a_max),
+                                          int(fill_radius), float(h), int(max_fill_passes)))
+
+
+def disc_mask_params(ctx, ct, cbct, stream=None):
+    """(Delta HU, HU_0, a_m, a_min, a_max) from the full-resolution images; synchronises"""
+    n = ctx.n(0)
+    out = (ctypes.c_float * 5)()
+    _check(ctx.handle, _lib.disc_mask_params(ctx.handle, _dev(ct, n), _dev(cbct, n), out, _stream(stream)))
+    return [float(v) for v in out]
+
+
+def disc_get_ab(ctx, level, out_a, out_b, out_xi, stream=None):
+    n = ctx.n(level)
+    xi_ptr = None
+    if out_xi is not None:
+        import torch
+        if not (out_xi.is_cuda and out_xi.dtype == torch.uint8 and out_xi.is_contiguous() and out_xi.numel() == n):
+            raise TypeError("out_xi: expected a contiguous uint8 CUDA tensor of the level's size")
+        xi_ptr = out_xi.data_ptr()
+    _check(ctx.handle, _lib.disc_get_ab(ctx.handle, level, _dev(out_a, n), _dev(out_b, n), xi_ptr, _stream(stream)))
+
+
+def disc_set_diagnostics(ctx, enable):
+    _check(ctx.handle, _lib.disc_set_diagnostics(ctx.handle, int(bool(enable))))
+
+
+def disc_get_diagnostics(ctx):
+    """(mean_a, mean_b), each a list of levels*iters floats, level-major from the coarsest level; synchronises"""
+    n = ctx.levels * max(ctx.iters, 1)
+    a, b = (ctypes.c_double * n)(), (ctypes.c_double * n)()
+    _check(ctx.handle, _lib.disc_get_diagnostics(ctx.handle, a, b))
+    return [float(v) for v in a], [float(v) for v in b]
 
 
 def disc_iterations_run(ctx):

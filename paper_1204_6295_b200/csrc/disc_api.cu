@@ -10,6 +10,7 @@
 
 #include "../../include/disc.h"
 #include "launch.h"
+#include "mask.cuh"
 #include "pyramid.cuh"
 
 using namespace disc;
@@ -26,6 +27,12 @@ struct Level {
     float* sp;       // corrected CBCT                                                   [N]
     float* disp;     // field of this level (levels >= 1; level 0 uses the caller's)     [3N]
     float* scratch;  // field after the x,y Gaussian passes                              [3N]
+    // NEXT-1 / diagnostics (allocated by disc_set_mask / disc_set_diagnostics)
+    float* mu_s;     // CBCT patch mean                                                  [N]
+    float* var_s;    // CBCT patch variance                                              [N]
+    float* A;        // a(x): E(M) while it is being computed                            [N]
+    float* B;        // b(x): VAR(M) while it is being computed                          [N]
+    unsigned char* xi;  // 0 free, 255 masked and unfilled, k = filled in pass k         [N bytes]
 };
 
 thread_local char g_create_error[256] = "";
@@ -47,6 +54,17 @@ struct disc_ctx {
     DevInfo di;       // device the context was created on, and its SM count
     GaussTaps taps;
     Level lv[DISC_MAX_LEVELS];
+    // NEXT-1: reliability mask and interpolation of a, b
+    int mask_on;
+    float mask_hu0, mask_a_min, mask_a_max;   // < 0: derived from the images
+    int fill_radius, max_fill_passes;
+    float fill_h;
+    int diag_on;      // Fig. 9 (e), (f): mean a, mean b per iteration
+    MaskCtl* d_mask;
+    double* d_partial;   // block partials of the deterministic reductions   [2 * kReduceBlocks]
+    double* d_mean_a;    // [levels * iters], level-major from the coarsest level
+    double* d_mean_b;
+    float* cbct_shift;   // CBCT + Delta HU at level 0                       [N_0]
     float* h2d_ct;    // device staging for disc_register_host
     float* h2d_cbct;
     float* d_out_disp;
@@ -86,6 +104,7 @@ disc_status check_launch(disc_ctx* c, const char* what) {
 bool level_ok(const disc_ctx* c, int level) { return level >= 0 && level < c->levels; }
 
 const IterCtl kNoCtl = {nullptr, 0};
+constexpr int kReduceBlocks = 592;   // grid of the grid-stride reductions (4 per SM on a B200)
 
 // every entry point runs on the device the context was created on (scratch, attributes and grid sizes belong to it)
 disc_status check_device(disc_ctx* c) {
@@ -146,10 +165,89 @@ disc_status launch_upsample(disc_ctx* c, const Level& coarse, const float* in, f
     return check_launch(c, "k_upsample_field");
 }
 
+
+// ---------------------------------------------------------------- NEXT-1 plumbing
+bool ab_path(const disc_ctx* c) { return c->mask_on || c->diag_on; }
+
+disc_status alloc_ab(disc_ctx* c) {
+    if (c->d_mask) return DISC_OK;
+    bool ok = cudaMalloc(&c->d_mask, sizeof(MaskCtl)) == cudaSuccess && cudaMemset(c->d_mask, 0, sizeof(MaskCtl)) == cudaSuccess &&
+              cudaMalloc(&c->d_partial, sizeof(double) * 2 * kReduceBlocks) == cudaSuccess;
+    const size_t nd = (size_t)c->levels * (c->iters > 0 ? c->iters : 1);
+    ok = ok && cudaMalloc(&c->d_mean_a, sizeof(double) * nd) == cudaSuccess && cudaMalloc(&c->d_mean_b, sizeof(double) * nd) == cudaSuccess &&
+         cudaMemset(c->d_mean_a, 0, sizeof(double) * nd) == cudaSuccess && cudaMemset(c->d_mean_b, 0, sizeof(double) * nd) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->cbct_shift, c->lv[0].N * sizeof(float)) == cudaSuccess;
+    for (int l = 0; ok && l < c->levels; ++l) {
+        Level& L = c->lv[l];
+        const size_t b = L.N * sizeof(float);
+        ok = cudaMalloc(&L.mu_s, b) == cudaSuccess && cudaMalloc(&L.var_s, b) == cudaSuccess && cudaMalloc(&L.A, b) == cudaSuccess &&
+             cudaMalloc(&L.B, b) == cudaSuccess && cudaMalloc(&L.xi, L.N) == cudaSuccess;
+    }
+    if (!ok) { cudaGetLastError(); return fail(c, DISC_ERR_ALLOC, "cudaMalloc failed (mask / diagnostics buffers)"); }
+    return DISC_OK;
+}
+
+unsigned reduce_grid(size_t N) {
+    const size_t b = (N + 255) / 256;
+    return (unsigned)(b < (size_t)kReduceBlocks ? b : (size_t)kReduceBlocks);
+}
+
+// the CBCT patch moments of a level (they never change within it)
+disc_status cache_cbct_moments(disc_ctx* c, const Level& L, const float* cbct, cudaStream_t st) {
+    return launch_moments<kModeMoments>(c, L, cbct, nullptr, L.mu_s, L.var_s, kNoCtl, st);
+}
+
+// A1 steps 1-3 with explicit a, b: moments of m, Eqs. (5)-(6), [Eq. (7), Eqs. (8)-(10)], a I_s + b.
+// out = nullptr: diagnostics only.  slot < 0: no diagnostics.
+disc_status correct_ab(disc_ctx* c, const Level& L, const float* cbct, const float* m, float* out, bool use_mask, int slot,
+                       IterCtl ctl, cudaStream_t st) {
+    DISC_TRY(launch_moments<kModeMoments>(c, L, m, nullptr, L.A, L.B, ctl, st));
+    const unsigned g = reduce_grid(L.N);
+    if (use_mask) {
+        k_fill_reset<<<1, 1, 0, st>>>(c->d_mask);
+        DISC_TRY(check_launch(c, "k_fill_reset"));
+        k_ab_mask<true><<<g, 256, 0, st>>>(m, cbct, L.mu_s, L.var_s, L.A, L.B, L.xi, L.N, DISC_EPS_VAR, c->d_mask);
+        DISC_TRY(check_launch(c, "k_ab_mask"));
+        dim3 grid((L.nx + 127) / 128, L.ny, L.nz);
+        const float inv_h2 = 1.f / (c->fill_h * c->fill_h);
+        for (int p = 1; p <= c->max_fill_passes; ++p) {
+            k_fill_pass<<<grid, 128, 0, st>>>(cbct, L.A, L.B, L.xi, L.nx, L.ny, L.nz, c->fill_radius, inv_h2, p, c->d_mask);
+            DISC_TRY(check_launch(c, "k_fill_pass"));
+        }
+    } else {
+        k_ab_mask<false><<<g, 256, 0, st>>>(m, cbct, L.mu_s, L.var_s, L.A, L.B, nullptr, L.N, DISC_EPS_VAR, c->d_mask);
+        DISC_TRY(check_launch(c, "k_ab"));
+    }
+    k_apply_ab<<<g, 256, 0, st>>>(cbct, L.A, L.B, out, L.N, c->d_partial, c->d_mask, slot >= 0 ? c->d_mean_a : nullptr,
+                                  c->d_mean_b, slot >= 0 ? slot : 0, ctl);
+    return check_launch(c, "k_apply_ab");
+}
+
+// Delta HU, HU_0 and (unless given) a_m, a_min, a_max from the two full-resolution images, into the device-side
+// MaskCtl.  `cbct` may be the unshifted image: the shift changes no variance.
+disc_status mask_parameters(disc_ctx* c, const float* ct, const float* cbct, cudaStream_t st) {
+    Level& L = c->lv[0];
+    if (cudaMemsetAsync(c->d_mask, 0, sizeof(MaskCtl), st) != cudaSuccess) return fail(c, DISC_ERR_CUDA, "cudaMemsetAsync failed");
+    k_sum2<<<reduce_grid(L.N), 256, 0, st>>>(ct, cbct, L.N, c->d_partial, c->d_mask, c->mask_hu0);
+    DISC_TRY(check_launch(c, "k_sum2"));
+    if (c->mask_a_min < 0.f) {
+        DISC_TRY(launch_moments<kModeMoments>(c, L, cbct, nullptr, L.mu_s, L.var_s, kNoCtl, st));
+        DISC_TRY(launch_moments<kModeMoments>(c, L, ct, nullptr, L.A, L.B, kNoCtl, st));     // r = 0: I_m = CT
+        for (int p = 0; p < 4; ++p) {
+            k_select_hist<<<reduce_grid(L.N), 256, 0, st>>>(L.var_s, L.B, L.N, DISC_EPS_VAR, p, c->d_mask);
+            DISC_TRY(check_launch(c, "k_select_hist"));
+            k_select_step<<<1, 1, 0, st>>>(p, c->d_mask);
+            DISC_TRY(check_launch(c, "k_select_step"));
+        }
+    }
+    k_mask_set<<<1, 1, 0, st>>>(c->d_mask, c->mask_hu0, c->mask_a_min, c->mask_a_max);
+    return check_launch(c, "k_mask_set");
+}
+
 // n_iters x { correct, force+update+Gxy, Gz+warp } on level L; on entry L.m must hold warp(ct, disp).
 // With final_warp the last iteration also refreshes L.m (needed when the caller goes on using it).
-disc_status iterate_level(disc_ctx* c, Level& L, const float* ct, float* disp, int n_iters, bool final_warp,
-                          cudaStream_t st) {
+disc_status iterate_level(disc_ctx* c, Level& L, const float* ct, const float* cbct, float* disp, int n_iters,
+                          bool final_warp, cudaStream_t st) {
     const int level = (int)(&L - c->lv);
     const bool stop = c->stop_eps >= 0.f;
     c->runs_host[level] = n_iters;
@@ -159,7 +257,13 @@ disc_status iterate_level(disc_ctx* c, Level& L, const float* ct, float* disp, i
         // with the criterion on, every kernel of iteration k falls through once an earlier iteration has tripped it;
         // the field and L.m then stay those of the last iteration run (its z pass always refreshes L.m: k + 1 < n_iters)
         const IterCtl ctl = stop ? IterCtl{&c->d_stop->stop_iter, k} : kNoCtl;
-        rc = launch_moments<kModeCorrect>(c, L, L.m, L.zhat, L.sp, nullptr, ctl, st);         // A1 steps 1,3
+        const int slot = c->diag_on && k < c->iters ? (c->levels - 1 - level) * c->iters + k : -1;
+        if (c->mask_on) {
+            rc = correct_ab(c, L, cbct, L.m, L.sp, true, slot, ctl, st);                       // A1 steps 1,2,3
+        } else {
+            rc = launch_moments<kModeCorrect>(c, L, L.m, L.zhat, L.sp, nullptr, ctl, st);     // A1 steps 1,3
+            if (rc == DISC_OK && slot >= 0) rc = correct_ab(c, L, cbct, L.m, nullptr, false, slot, ctl, st);   // Fig. 9 only
+        }
         if (rc == DISC_OK && stop) {                                                           // PAPER.md:167, l^(k)
             launch_force_norms(c->force_mode, L.m, L.sp, disp, L.nx, L.ny, L.nz, DISC_EPS_DEN, c->d_stop, k, c->stop_eps,
                                c->di.n_sm, st);
@@ -182,7 +286,9 @@ void free_ctx(disc_ctx* c) {
         Level& L = c->lv[l];
         cudaFree(L.ct); cudaFree(L.cbct); cudaFree(L.zhat); cudaFree(L.m); cudaFree(L.sp);
         cudaFree(L.disp); cudaFree(L.scratch);
+        cudaFree(L.mu_s); cudaFree(L.var_s); cudaFree(L.A); cudaFree(L.B); cudaFree(L.xi);
     }
+    cudaFree(c->d_mask); cudaFree(c->d_partial); cudaFree(c->d_mean_a); cudaFree(c->d_mean_b); cudaFree(c->cbct_shift);
     cudaFree(c->d_stop);
     cudaFree(c->h2d_ct); cudaFree(c->h2d_cbct); cudaFree(c->d_out_disp); cudaFree(c->d_out_corr);
     delete c;
@@ -317,6 +423,86 @@ disc_status disc_iterations_run(disc_ctx* c, int* out_host) {
     return DISC_OK;
 }
 
+disc_status disc_set_mask(disc_ctx* c, int enable, float hu0, float a_min, float a_max, int fill_radius, float h,
+                          int max_fill_passes) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
+    if (!enable) { c->mask_on = 0; return DISC_OK; }
+    DISC_NEED(c, hu0 == hu0 && a_min == a_min && a_max == a_max && h == h, "NaN parameter");
+    DISC_NEED(c, a_min < 0.f || a_max >= a_min, "a_max < a_min");
+    DISC_NEED(c, fill_radius >= 1 && fill_radius <= 8, "fill_radius must be in 1..8");
+    DISC_NEED(c, h > 0.f, "h <= 0");
+    DISC_NEED(c, max_fill_passes >= 1 && max_fill_passes <= 254, "max_fill_passes must be in 1..254");
+    DISC_TRY(alloc_ab(c));
+    c->mask_on = 1;
+    c->mask_hu0 = hu0 >= 0.f ? hu0 : -1.f;
+    c->mask_a_min = a_min >= 0.f ? a_min : -1.f;
+    c->mask_a_max = a_min >= 0.f ? a_max : -1.f;
+    c->fill_radius = fill_radius; c->fill_h = h; c->max_fill_passes = max_fill_passes;
+    // the given parameters go to the device-side control block now, so that the fine-grained calls can be used without
+    // disc_mask_params / disc_register; the derived ones are (re)computed there by those two
+    MaskCtl h0;
+    std::memset(&h0, 0, sizeof(h0));
+    h0.hu0 = hu0 >= 0.f ? hu0 : 0.f;
+    h0.a_m = 1.f;
+    h0.a_min = a_min >= 0.f ? a_min : 0.5f;
+    h0.a_max = a_min >= 0.f ? a_max : 1.5f;
+    if (cudaMemcpy(c->d_mask, &h0, sizeof(h0), cudaMemcpyHostToDevice) != cudaSuccess)
+        return fail(c, DISC_ERR_CUDA, "cudaMemcpy (mask parameters) failed");
+    return DISC_OK;
+}
+
+disc_status disc_mask_params(disc_ctx* c, const float* ct, const float* cbct, float out_host[5], void* stream) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
+    DISC_NEED(c, c->mask_on, "the mask is off (disc_set_mask)");
+    DISC_NEED(c, ct && cbct && out_host, "NULL pointer");
+    cudaStream_t st = (cudaStream_t)stream;
+    DISC_TRY(mask_parameters(c, ct, cbct, st));
+    MaskCtl h;
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaMemcpy(&h, c->d_mask, sizeof(h), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return fail(c, DISC_ERR_CUDA, "reading the mask parameters: %s", cudaGetErrorString(e));
+    out_host[0] = (float)h.delta_hu; out_host[1] = h.hu0; out_host[2] = h.a_m; out_host[3] = h.a_min; out_host[4] = h.a_max;
+    return DISC_OK;
+}
+
+disc_status disc_get_ab(disc_ctx* c, int level, float* out_a, float* out_b, unsigned char* out_xi, void* stream) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
+    DISC_NEED(c, level_ok(c, level), "level out of range");
+    DISC_NEED(c, c->d_mask, "neither the mask nor the diagnostics are on");
+    const Level& L = c->lv[level];
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = cudaSuccess;
+    if (out_a) e = cudaMemcpyAsync(out_a, L.A, L.N * sizeof(float), cudaMemcpyDeviceToDevice, st);
+    if (e == cudaSuccess && out_b) e = cudaMemcpyAsync(out_b, L.B, L.N * sizeof(float), cudaMemcpyDeviceToDevice, st);
+    if (e == cudaSuccess && out_xi) e = cudaMemcpyAsync(out_xi, L.xi, L.N, cudaMemcpyDeviceToDevice, st);
+    if (e != cudaSuccess) return fail(c, DISC_ERR_CUDA, "copy failed: %s", cudaGetErrorString(e));
+    return DISC_OK;
+}
+
+disc_status disc_set_diagnostics(disc_ctx* c, int enable) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
+    if (enable) DISC_TRY(alloc_ab(c));
+    c->diag_on = enable ? 1 : 0;
+    return DISC_OK;
+}
+
+disc_status disc_get_diagnostics(disc_ctx* c, double* mean_a_host, double* mean_b_host) {
+    if (!c) return DISC_ERR_INVALID_ARG;
+    DISC_TRY(check_device(c));
+    DISC_NEED(c, c->diag_on && c->d_mean_a, "the diagnostics are off (disc_set_diagnostics)");
+    DISC_NEED(c, mean_a_host && mean_b_host, "NULL pointer");
+    const size_t nd = (size_t)c->levels * (c->iters > 0 ? c->iters : 1) * sizeof(double);
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpy(mean_a_host, c->d_mean_a, nd, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(mean_b_host, c->d_mean_b, nd, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return fail(c, DISC_ERR_CUDA, "reading the diagnostics: %s", cudaGetErrorString(e));
+    return DISC_OK;
+}
+
 disc_status disc_warp(disc_ctx* c, int level, const float* moving, const float* disp, float* out, void* stream) {
     if (!c) return DISC_ERR_INVALID_ARG;
     DISC_TRY(check_device(c));
@@ -333,6 +519,10 @@ disc_status disc_correct_intensity(disc_ctx* c, int level, const float* cbct, co
     DISC_NEED(c, cbct && ct_warped && out_corrected, "NULL pointer");
     Level& L = c->lv[level];
     cudaStream_t st = (cudaStream_t)stream;
+    if (c->mask_on) {   // Eqs. (5)-(10) with the mask parameters the context holds (disc_set_mask / disc_mask_params)
+        DISC_TRY(cache_cbct_moments(c, L, cbct, st));
+        return correct_ab(c, L, cbct, ct_warped, out_corrected, true, -1, kNoCtl, st);
+    }
     DISC_TRY(launch_moments<kModeZscore>(c, L, cbct, nullptr, L.zhat, nullptr, kNoCtl, st));
     return launch_moments<kModeCorrect>(c, L, ct_warped, L.zhat, out_corrected, nullptr, kNoCtl, st);
 }
@@ -358,9 +548,10 @@ disc_status disc_iterate(disc_ctx* c, int level, const float* ct, const float* c
     DISC_NEED(c, n_iters >= 0, "n_iters < 0");
     Level& L = c->lv[level];
     cudaStream_t st = (cudaStream_t)stream;
-    DISC_TRY(launch_moments<kModeZscore>(c, L, cbct, nullptr, L.zhat, nullptr, kNoCtl, st));
+    if (!c->mask_on) DISC_TRY(launch_moments<kModeZscore>(c, L, cbct, nullptr, L.zhat, nullptr, kNoCtl, st));
+    if (ab_path(c)) DISC_TRY(cache_cbct_moments(c, L, cbct, st));
     DISC_TRY(launch_warp(c, L, ct, disp_inout, L.m, st));
-    return iterate_level(c, L, ct, disp_inout, n_iters, true, st);
+    return iterate_level(c, L, ct, cbct, disp_inout, n_iters, true, st);
 }
 
 disc_status disc_profile_iteration(disc_ctx* c, int level, const float* ct, const float* cbct, float* disp_inout,
@@ -415,6 +606,13 @@ disc_status disc_register(disc_ctx* c, const float* ct, const float* cbct, float
     const float* pct[DISC_MAX_LEVELS];
     const float* pcb[DISC_MAX_LEVELS];
     pct[0] = ct; pcb[0] = cbct;
+    if (c->mask_on) {
+        // A1 "Globally adjust the intensity of CBCT" and the mask parameters
+        DISC_TRY(mask_parameters(c, ct, cbct, st));
+        k_shift<<<reduce_grid(c->lv[0].N), 256, 0, st>>>(cbct, c->cbct_shift, c->lv[0].N, c->d_mask);
+        DISC_TRY(check_launch(c, "k_shift"));
+        pcb[0] = c->cbct_shift;
+    }
     for (int l = 1; l < nl; ++l) {
         DISC_TRY(launch_downsample(c, c->lv[l - 1], pct[l - 1], c->lv[l].ct, st));
         DISC_TRY(launch_downsample(c, c->lv[l - 1], pcb[l - 1], c->lv[l].cbct, st));
@@ -429,12 +627,15 @@ disc_status disc_register(disc_ctx* c, const float* ct, const float* cbct, float
         } else {
             DISC_TRY(launch_upsample(c, c->lv[l + 1], c->lv[l + 1].disp, r, st));
         }
-        DISC_TRY(launch_moments<kModeZscore>(c, L, pcb[l], nullptr, L.zhat, nullptr, kNoCtl, st));
+        if (!c->mask_on) DISC_TRY(launch_moments<kModeZscore>(c, L, pcb[l], nullptr, L.zhat, nullptr, kNoCtl, st));
+        if (ab_path(c)) DISC_TRY(cache_cbct_moments(c, L, pcb[l], st));
         DISC_TRY(launch_warp(c, L, pct[l], r, L.m, st));
         const bool need_m = (l == 0 && out_corrected_cbct != nullptr);
-        DISC_TRY(iterate_level(c, L, pct[l], r, c->iters, need_m, st));
-        if (need_m)                                                                    // reading A12
-            DISC_TRY(launch_moments<kModeCorrect>(c, L, L.m, L.zhat, out_corrected_cbct, nullptr, kNoCtl, st));
+        DISC_TRY(iterate_level(c, L, pct[l], pcb[l], r, c->iters, need_m, st));
+        if (need_m) {                                                                  // reading A12
+            if (c->mask_on) DISC_TRY(correct_ab(c, L, pcb[l], L.m, out_corrected_cbct, true, -1, kNoCtl, st));
+            else DISC_TRY(launch_moments<kModeCorrect>(c, L, L.m, L.zhat, out_corrected_cbct, nullptr, kNoCtl, st));
+        }
     }
     return DISC_OK;
 }

@@ -1,0 +1,291 @@
+// mask.cuh -- SURVEY NEXT-1: the paper's reliability mask and the interpolation / extrapolation of a, b
+// (Eqs. (5)-(10); parameters PAPER.md:161, :165), plus the Fig.-9 averages of a and b
+// (PAPER.md:398-402).  Everything is decided on the device: the parameters (Delta HU, HU_0, a_m, a_min, a_max) live in
+// a MaskCtl in device memory that the kernels read, the fill passes stop through a device-side counter, so the
+// registration still enqueues its whole schedule without a host synchronisation.
+//
+//   k_sum2            sum(ct), sum(cbct) -> Delta HU = mean(ct) - mean(cbct), HU_0 = 2 |Delta HU|
+//   k_shift           cbct + Delta HU  ("globally adjust the intensity of CBCT", Alg. A1)
+//   k_ab_mask         a = STD(M)/STD(S), b = E(M) - a E(S); xi by Eq. (7); a = b = 0 where xi = 1
+//   k_select_*        a_m = lower median of a over the voxels with both variances > eps (radix select)
+//   k_fill_pass       Eqs. (8)-(10), one Jacobi pass over the cube T
+//   k_apply_ab        I'_s = a I_s + b, and the sums of a and b
+#pragma once
+#include <float.h>
+
+#include "common.cuh"
+
+namespace disc {
+
+constexpr unsigned char kXiFree = 0;        // xi = 0: a, b from Eqs. (5)-(6)
+constexpr unsigned char kXiMasked = 255;    // xi = 1 and not filled yet; 1..254: filled in that pass
+
+struct MaskCtl {
+    double sum_ct, sum_cbct;     // k_sum2 accumulators (block partials added in block order by the last block)
+    double delta_hu;             // mean(ct) - mean(cbct)
+    float hu0, a_m, a_min, a_max;
+    // radix select of the median
+    unsigned hist[256];
+    unsigned long long count;    // qualifying voxels
+    unsigned long long rank;     // remaining rank inside the current prefix
+    unsigned prefix;             // bits of the median fixed so far
+    // fill passes
+    unsigned remaining, filled, prev_filled, ticket;
+    // diagnostics of the running iteration
+    double sum_a, sum_b;
+    unsigned ticket2;
+};
+
+// ---------------------------------------------------------------- Delta HU
+// Deterministic two-stage sum: every block writes its partial, the last block to finish adds them in block order.
+static __global__ void __launch_bounds__(256)
+k_sum2(const float* __restrict__ ct, const float* __restrict__ cbct, size_t N, double* __restrict__ partial, MaskCtl* ctl,
+       float hu0_fixed) {
+    double a = 0.0, b = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
+        a += (double)__ldg(ct + i);
+        b += (double)__ldg(cbct + i);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); b += __shfl_xor_sync(0xffffffffu, b, o); }
+    __shared__ double sh[2][8];
+    __shared__ bool last;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) { sh[0][warp] = a; sh[1][warp] = b; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double ta = 0.0, tb = 0.0;
+        for (int w = 0; w < 8; ++w) { ta += sh[0][w]; tb += sh[1][w]; }
+        partial[2 * blockIdx.x] = ta; partial[2 * blockIdx.x + 1] = tb;
+        __threadfence();
+        last = atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (last && threadIdx.x == 0) {
+        __threadfence();
+        double ta = 0.0, tb = 0.0;
+        for (unsigned k = 0; k < gridDim.x; ++k) { ta += partial[2 * k]; tb += partial[2 * k + 1]; }
+        ctl->sum_ct = ta; ctl->sum_cbct = tb;
+        ctl->delta_hu = (ta - tb) / (double)N;
+        ctl->hu0 = hu0_fixed >= 0.f ? hu0_fixed : (float)(2.0 * fabs(ctl->delta_hu));
+        ctl->ticket = 0u;
+    }
+}
+
+static __global__ void __launch_bounds__(256)
+k_shift(const float* __restrict__ in, float* __restrict__ out, size_t N, const MaskCtl* __restrict__ ctl) {
+    const double d = ctl->delta_hu;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x)
+        out[i] = (float)((double)__ldg(in + i) + d);
+}
+
+static __global__ void k_mask_set(MaskCtl* ctl, float hu0, float a_min, float a_max) {
+    if (hu0 >= 0.f) ctl->hu0 = hu0;
+    if (a_min >= 0.f) { ctl->a_min = a_min; ctl->a_max = a_max; }
+}
+
+// ---------------------------------------------------------------- a, b and the mask
+// In place: A holds E(M) on entry and a on exit, B holds VAR(M) on entry and b on exit.  With USE_MASK = false only
+// Eqs. (5)-(6) are evaluated (xi = 0 everywhere): that is what the median of A before the DIR and the diagnostics of
+// the unmasked path use.
+template <bool USE_MASK>
+__global__ void __launch_bounds__(256)
+k_ab_mask(const float* __restrict__ m, const float* __restrict__ cbct, const float* __restrict__ mu_s,
+          const float* __restrict__ var_s, float* __restrict__ A, float* __restrict__ B, unsigned char* __restrict__ xi,
+          size_t N, float eps_var, MaskCtl* ctl) {
+    const float hu0 = ctl->hu0, a_min = ctl->a_min, a_max = ctl->a_max;
+    unsigned masked = 0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
+        const float mu_m = A[i], var_m = B[i], vs = __ldg(var_s + i);
+        const float a = vs > eps_var ? sqrtf(var_m / vs) : 0.f;          // Eq. (5); reading A5
+        const float b = fmaf(-a, __ldg(mu_s + i), mu_m);                 // Eq. (6)
+        bool x = false;
+        if (USE_MASK) {
+            // Eq. (7): the difference of two fp32 values is taken in fp64 (exact), as is the comparison
+            const double d = fabs((double)__ldg(m + i) - (double)__ldg(cbct + i));
+            x = d > (double)hu0 || a < a_min || a > a_max;
+        }
+        A[i] = x ? 0.f : a;                                              // "Initially a = b = 0 for xi = 1"
+        B[i] = x ? 0.f : b;
+        if (xi) xi[i] = x ? kXiMasked : kXiFree;
+        masked += x ? 1u : 0u;
+    }
+    if (USE_MASK) {
+        masked = __reduce_add_sync(0xffffffffu, masked);
+        if ((threadIdx.x & 31) == 0 && masked) atomicAdd(&ctl->remaining, masked);
+    }
+}
+
+// ---------------------------------------------------------------- median of A (reading A17)
+// 4 passes of an 8-bit radix select on the bit pattern of a >= 0 (monotonic), over the voxels where Eq. (5) is a ratio of
+// two positive deviations.  pass = 0 also counts the qualifying voxels.
+static __global__ void __launch_bounds__(256)
+k_select_hist(const float* __restrict__ var_s, const float* __restrict__ var_m, size_t N, float eps_var, int pass,
+              MaskCtl* ctl) {
+    __shared__ unsigned h[256];
+    h[threadIdx.x] = 0u;
+    __syncthreads();
+    const unsigned prefix = ctl->prefix;
+    const int shift = 24 - 8 * pass;
+    const unsigned himask = pass == 0 ? 0u : 0xffffffffu << (shift + 8);
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
+        const float vs = __ldg(var_s + i), vm = __ldg(var_m + i);
+        if (!(vs > eps_var && vm > eps_var)) continue;
+        const unsigned bits = __float_as_uint(sqrtf(vm / vs));          // Eq. (5), the same expression as k_ab_mask
+        if ((bits & himask) == (prefix & himask)) atomicAdd(&h[(bits >> shift) & 255u], 1u);
+    }
+    __syncthreads();
+    if (h[threadIdx.x]) atomicAdd(&ctl->hist[threadIdx.x], h[threadIdx.x]);
+}
+
+static __global__ void k_select_step(int pass, MaskCtl* ctl) {
+    if (pass == 0) {
+        unsigned long long n = 0;
+        for (int b = 0; b < 256; ++b) n += ctl->hist[b];
+        ctl->count = n;
+        ctl->rank = n ? (n - 1) / 2 : 0;                                 // lower median
+    }
+    unsigned long long r = ctl->rank;
+    int b = 0;
+    if (ctl->count) {
+        for (; b < 255; ++b) {
+            if (r < ctl->hist[b]) break;
+            r -= ctl->hist[b];
+        }
+    }
+    ctl->rank = r;
+    ctl->prefix |= (unsigned)b << (24 - 8 * pass);
+    for (int k = 0; k < 256; ++k) ctl->hist[k] = 0u;
+    if (pass == 3) {
+        ctl->a_m = ctl->count ? __uint_as_float(ctl->prefix) : 1.f;      // no qualifying voxel: a_m = 1
+        ctl->a_min = 0.5f * ctl->a_m;
+        ctl->a_max = 1.5f * ctl->a_m;
+        ctl->prefix = 0u;
+    }
+}
+
+// ---------------------------------------------------------------- Eqs. (8)-(10)
+// One Jacobi pass `pass` (1..254): a voxel with xi = masked looks at the voxels of T (cube of radius rt, truncated to
+// the volume) that were available before this pass (stamp < pass), takes w = exp(-((D)^2 - min D^2) / h^2) (the same
+// quotient as Eqs. (8)-(9), normalised by the largest weight so that it cannot underflow to 0/0) and, if there is one,
+// writes its a, b and stamps itself with `pass`.  Stamps written in this pass are >= pass, so nobody reads them in this
+// pass: the update is in place and race free.  The last block rolls the counters; when nothing is left, or a pass
+// filled nothing, the remaining passes fall through.
+static __global__ void __launch_bounds__(128)
+k_fill_pass(const float* __restrict__ cbct, float* __restrict__ A, float* __restrict__ B, unsigned char* __restrict__ xi,
+            int nx, int ny, int nz, int rt, float inv_h2, int pass, MaskCtl* ctl) {
+    {
+        const volatile MaskCtl* c = ctl;
+        if (c->remaining == 0u || (pass > 1 && c->prev_filled == 0u)) return;
+    }
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y, z = blockIdx.z;
+    unsigned mine = 0;
+    if (x < nx) {
+        const size_t i0 = ((size_t)z * ny + y) * nx + x;
+        if (xi[i0] == kXiMasked) {
+            const float s0 = __ldg(cbct + i0);
+            const int xa = max(x - rt, 0), xb = min(x + rt, nx - 1);
+            const int ya = max(y - rt, 0), yb = min(y + rt, ny - 1);
+            const int za = max(z - rt, 0), zb = min(z + rt, nz - 1);
+            float dmin = FLT_MAX;
+            for (int c = za; c <= zb; ++c)
+                for (int b = ya; b <= yb; ++b) {
+                    const size_t row = ((size_t)c * ny + b) * nx;
+                    for (int a = xa; a <= xb; ++a) {
+                        if (xi[row + a] >= pass) continue;
+                        const float d = __ldg(cbct + row + a) - s0;
+                        dmin = fminf(dmin, d * d);
+                    }
+                }
+            if (dmin < FLT_MAX) {
+                float sw = 0.f, sa = 0.f, sb = 0.f;
+                for (int c = za; c <= zb; ++c)
+                    for (int b = ya; b <= yb; ++b) {
+                        const size_t row = ((size_t)c * ny + b) * nx;
+                        for (int a = xa; a <= xb; ++a) {
+                            if (xi[row + a] >= pass) continue;
+                            const float d = __ldg(cbct + row + a) - s0;
+                            const float w = __expf(-(d * d - dmin) * inv_h2);      // Eq. (10)
+                            sw += w;
+                            sa = fmaf(w, A[row + a], sa);
+                            sb = fmaf(w, B[row + a], sb);
+                        }
+                    }
+                A[i0] = sa / sw;                                                   // Eqs. (8), (9)
+                B[i0] = sb / sw;
+                __threadfence();
+                xi[i0] = (unsigned char)pass;
+                mine = 1u;
+            }
+        }
+    }
+    mine = __reduce_add_sync(0xffffffffu, mine);
+    __shared__ unsigned blk;
+    __shared__ bool last;
+    if (threadIdx.x == 0) blk = 0u;
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0 && mine) atomicAdd(&blk, mine);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        if (blk) atomicAdd(&ctl->filled, blk);
+        __threadfence();
+        const unsigned total = gridDim.x * gridDim.y * gridDim.z;
+        last = atomicAdd(&ctl->ticket, 1u) == total - 1;
+        if (last) {
+            __threadfence();
+            const unsigned f = atomicAdd(&ctl->filled, 0u);
+            ctl->remaining -= f;
+            ctl->prev_filled = f;
+            ctl->filled = 0u;
+            ctl->ticket = 0u;
+            __threadfence();
+        }
+    }
+}
+
+static __global__ void k_fill_reset(MaskCtl* ctl) {
+    ctl->remaining = 0u; ctl->filled = 0u; ctl->prev_filled = 0u; ctl->ticket = 0u;
+}
+
+// ---------------------------------------------------------------- I'_s = a I_s + b and Fig. 9 (e), (f)
+// out may be NULL (diagnostics only).  diag (may be NULL): [0] += sum a, [1] += sum b of this iteration, through block
+// partials added in block order by the last block (deterministic); slot = where the two averages are filed.
+static __global__ void __launch_bounds__(256)
+k_apply_ab(const float* __restrict__ cbct, const float* __restrict__ A, const float* __restrict__ B,
+           float* __restrict__ out, size_t N, double* __restrict__ partial, MaskCtl* ctl, double* __restrict__ mean_a,
+           double* __restrict__ mean_b, int slot, IterCtl ictl) {
+    if (iter_skipped(ictl)) return;
+    double sa = 0.0, sb = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
+        const float a = A[i], b = B[i];
+        if (out) out[i] = fmaf(a, __ldg(cbct + i), b);
+        sa += (double)a; sb += (double)b;
+    }
+    if (!mean_a) return;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { sa += __shfl_xor_sync(0xffffffffu, sa, o); sb += __shfl_xor_sync(0xffffffffu, sb, o); }
+    __shared__ double sh[2][8];
+    __shared__ bool last;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) { sh[0][warp] = sa; sh[1][warp] = sb; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double ta = 0.0, tb = 0.0;
+        for (int w = 0; w < 8; ++w) { ta += sh[0][w]; tb += sh[1][w]; }
+        partial[2 * blockIdx.x] = ta; partial[2 * blockIdx.x + 1] = tb;
+        __threadfence();
+        last = atomicAdd(&ctl->ticket2, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (last && threadIdx.x == 0) {
+        __threadfence();
+        double ta = 0.0, tb = 0.0;
+        for (unsigned k = 0; k < gridDim.x; ++k) { ta += partial[2 * k]; tb += partial[2 * k + 1]; }
+        mean_a[slot] = ta / (double)N;
+        mean_b[slot] = tb / (double)N;
+        ctl->ticket2 = 0u;
+    }
+}
+
+}  // namespace disc
