@@ -35,6 +35,9 @@ KERNELS = (
 )
 
 
+ITER_BPV = sum(b for _, b in KERNELS)
+
+
 def schedule_voxel_updates(dims, levels, iters):
     nx, ny, nz = dims
     return sum((nx >> l) * (ny >> l) * (nz >> l) * iters for l in range(levels))
@@ -94,7 +97,9 @@ class ClockSampler:
 
 
 def oracle_sample(ct, cbct, R, sigma, n_iter):
-    """n_iter finest-level iterations of the oracle as it stands (stepwise functions), timed on the host cores."""
+    """n_iter finest-level iterations of the oracle as it stands (stepwise functions), timed on the host cores.  The
+    CBCT patch moments are computed once per level in the schedule (1/100 of it) and stay OUTSIDE the clock, here and
+    in --impl reference alike, so that the two CPU numbers are the same measurement."""
     import numpy as np
     import oracle
     r = np.zeros((3,) + ct.shape, dtype=np.float32)
@@ -117,14 +122,15 @@ def run_reference(args):
     import phantoms
     ct, cbct, _, p = phantoms.make_pair(WORKLOAD_CONFIG)
     R, sigma = p["patch_radius"], p["sigma"]
-    sample = "1 finest-level iteration (256x256x128, R=5, sigma=2) of the config-3 schedule per step"
+    sample = ("1 finest-level iteration (256x256x128, R=5, sigma=2) of the config-3 schedule per step; the per-level "
+              "CBCT moments (1/100 of a level) are outside the clock, as in cpu_baseline")
     for _ in range(args.warmup):
         oracle_sample(ct, cbct, R, sigma, 1)
-    t0 = time.perf_counter()
+    dt = 0.0
     cores = 1
     for _ in range(args.steps):
-        _, _, cores = oracle_sample(ct, cbct, R, sigma, 1)
-    dt = time.perf_counter() - t0
+        _, d, cores = oracle_sample(ct, cbct, R, sigma, 1)
+        dt += d
     value = ct.size * args.steps / dt
     line = {
         "impl": "reference", "metric": "voxel_updates_per_sec", "value": value, "unit": "voxel-updates/s",
@@ -309,6 +315,46 @@ def main():
     torch.cuda.synchronize()
     ms_stop, runs_stop = f0.elapsed_time(f1), disc.disc_iterations_run(ctx)
     disc.disc_set_stop(ctx, -1.0)
+    # per-level steady-state iteration time (coarse levels are latency-bound: SURVEY H5)
+    us_per_level = []
+    for l in range(levels):
+        ld = ctx.level_dims(l)
+        a = torch.zeros((ld[2], ld[1], ld[0]), device="cuda").normal_(0.0, 300.0)
+        b = torch.zeros_like(a).normal_(0.0, 300.0)
+        rr = torch.zeros((3, ld[2], ld[1], ld[0]), device="cuda")
+        disc.disc_iterate(ctx, l, a, b, rr, 5)
+        torch.cuda.synchronize()
+        f0.record(stream)
+        disc.disc_iterate(ctx, l, a, b, rr, 100)
+        f1.record(stream)
+        torch.cuda.synchronize()
+        us_per_level.append(10.0 * f0.elapsed_time(f1))
+        del a, b, rr
+    # the same registration with the paper's reliability mask and interpolation of a, b
+    disc.disc_set_mask(ctx, True, fill_radius=1, h=50.0, max_fill_passes=8)
+    disc.disc_register(ctx, d_ct, d_cb, d_r2, d_corr)
+    torch.cuda.synchronize()
+    f0.record(stream)
+    disc.disc_register(ctx, d_ct, d_cb, d_r2, d_corr)
+    f1.record(stream)
+    torch.cuda.synchronize()
+    ms_mask = f0.elapsed_time(f1)
+    mask_params = disc.disc_mask_params(ctx, d_ct, d_cb)
+    disc.disc_set_mask(ctx, False)
+    # the paper's clinical geometry (256x256x68, patch 3x3x3, two levels, transverse plane halved only)
+    cct, ccb, _, _ = phantoms.make_pair(3, dims=(256, 256, 68))
+    cctx = disc.disc_create_ex((256, 256, 68), (0.94, 0.94, 2.5), (1, 1, 1), 2.0, 2, 100, (2, 2, 1))
+    c_ct, c_cb = torch.from_numpy(cct).cuda(), torch.from_numpy(ccb).cuda()
+    c_r, c_corr = torch.empty((3, 68, 256, 256), device="cuda"), torch.empty((68, 256, 256), device="cuda")
+    disc.disc_register(cctx, c_ct, c_cb, c_r, c_corr)
+    torch.cuda.synchronize()
+    f0.record(stream)
+    disc.disc_register(cctx, c_ct, c_cb, c_r, c_corr)
+    f1.record(stream)
+    torch.cuda.synchronize()
+    ms_clinical = f0.elapsed_time(f1)
+    disc.disc_destroy(cctx)
+    del c_ct, c_cb, c_r, c_corr
     clocks = sampler.stop() if rank == 0 else None
 
     # ---------------- end to end: pinned host buffers through disc_register_host
@@ -343,20 +389,26 @@ def main():
         gbs = bpv * n0 / (ms * 1e-3) / 1e9
         per_kernel.append({"kernel": name, "ms": ms, "bytes_per_voxel": bpv, "gbs": gbs, "frac": gbs / peak})
     dom = max(per_kernel, key=lambda k: k["ms"])
-    traffic = None                                              # dram bytes per launch from the latest `ncu --set full`
-    tpath = os.path.join(ROOT, "profiles", "r01c_traffic.csv")  # capture (profiles/r01c_launches_and_ncu.md), text only
+    # DRAM bytes per launch are not measurable inside this run (no profiler here): they come from the committed
+    # `ncu --set full` capture of the SAME kernels, and the line says which capture and which commit it belongs to
+    traffic, traffic_source = None, None
+    tpath = os.path.join(ROOT, "profiles", "r02_traffic.csv")
     if os.path.exists(tpath):
         try:
-            for ln in open(tpath).read().splitlines()[1:]:
+            lines = open(tpath).read().splitlines()
+            traffic_source = lines[0].lstrip("# ").strip()
+            for ln in lines[2:]:
                 f = ln.split(",")
                 if f[0] == dom["kernel"]:
                     traffic = float(f[1])
         except Exception:
-            traffic = None
+            traffic, traffic_source = None, None
     roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["gbs"], "peak": peak, "unit": "GB/s",
-                "frac": dom["gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
+                "frac": dom["gbs"] / peak, "frac_of_nominal_8tbs": dom["gbs"] / 8000.0, "traffic": traffic,
+                "traffic_source": traffic_source, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": dom["bytes_per_voxel"] * n0, "per_kernel": per_kernel,
-                "iteration_gbs": 76.0 * n0 / (ms_iter * 1e-3) / 1e9, "iteration_frac": 76.0 * n0 / (ms_iter * 1e-3) / 1e9 / peak}
+                "iteration_bytes_per_voxel": ITER_BPV, "iteration_gbs": ITER_BPV * n0 / (ms_iter * 1e-3) / 1e9,
+                "iteration_frac": ITER_BPV * n0 / (ms_iter * 1e-3) / 1e9 / peak}
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -376,6 +428,12 @@ def main():
         "ms_per_iteration_finest": ms_iter,
         "double_force": {"ms_per_iteration_finest": ms_iter_double, "iterations_per_s_finest": 1e3 / ms_iter_double},
         "stopping_criterion": {"eps": 1e-4, "iterations_run_per_level": runs_stop, "ms_per_registration": ms_stop},
+        "us_per_iteration_per_level": us_per_level,
+        "mask_and_interpolation": {"ms_per_registration": ms_mask, "fill_radius": 1, "h": 50.0, "max_fill_passes": 8,
+                                   "delta_hu": mask_params[0], "hu0": mask_params[1], "a_m": mask_params[2]},
+        "clinical_geometry": {"workload": "256x256x68 (0.94x0.94x2.5 mm), patch 3x3x3, 2 levels halving x,y only, "
+                                          "100 iters/level (PAPER.md:236, :382, :412: 69 s on a Tesla C1060)",
+                              "ms_per_registration": ms_clinical},
         "e2e": {"value": e2e_value, "unit": "voxel-updates/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": ms_e2e / n_e2e},
         "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,

@@ -19,8 +19,9 @@ struct Dims {
 // Stopping criterion: device-side state of one context.  Every kernel of iteration
 // `iter` gets an IterCtl by value and returns at once when iter > *stop_iter, so an early stop needs no host
 // synchronisation: the remaining launches of the level fall through.  stop_iter == nullptr: criterion off.
+constexpr int kStopBlocks = 2048;   // most blocks k_force_norms is launched with
 struct StopCtl {
-    double sum_dr, sum_r;      // accumulators of the running iteration
+    double partial[2 * kStopBlocks];   // per-block (sum|dr|, sum|r|) of the running iteration, added in block order
     double hist[16];           // l^(k) of the last 16 iterations, slot k & 15
     unsigned ticket;           // blocks of k_force_norms finished
     int stop_iter;             // last iteration of the level (INT_MAX while running)

@@ -412,11 +412,11 @@ disc_status disc_iterations_run(disc_ctx* c, int* out_host) {
     if (!c) return DISC_ERR_INVALID_ARG;
     DISC_NEED(c, out_host, "NULL pointer");
     if (c->stop_eps >= 0.f) {
-        StopCtl h;
+        int runs[DISC_MAX_LEVELS];
         cudaError_t e = cudaDeviceSynchronize();
-        if (e == cudaSuccess) e = cudaMemcpy(&h, c->d_stop, sizeof(h), cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess) e = cudaMemcpy(runs, c->d_stop->runs, sizeof(runs), cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) return fail(c, DISC_ERR_CUDA, "reading the stop control: %s", cudaGetErrorString(e));
-        for (int l = 0; l < c->levels; ++l) out_host[l] = h.runs[l];
+        for (int l = 0; l < c->levels; ++l) out_host[l] = runs[l];
     } else {
         for (int l = 0; l < c->levels; ++l) out_host[l] = c->runs_host[l];
     }
@@ -548,6 +548,10 @@ disc_status disc_iterate(disc_ctx* c, int level, const float* ct, const float* c
     DISC_NEED(c, n_iters >= 0, "n_iters < 0");
     Level& L = c->lv[level];
     cudaStream_t st = (cudaStream_t)stream;
+    // only this level runs: the counts of the others read 0
+    for (int l = 0; l < DISC_MAX_LEVELS; ++l) c->runs_host[l] = 0;
+    if (c->stop_eps >= 0.f && cudaMemsetAsync(c->d_stop->runs, 0, sizeof(c->d_stop->runs), st) != cudaSuccess)
+        return fail(c, DISC_ERR_CUDA, "cudaMemsetAsync failed");
     if (!c->mask_on) DISC_TRY(launch_moments<kModeZscore>(c, L, cbct, nullptr, L.zhat, nullptr, kNoCtl, st));
     if (ab_path(c)) DISC_TRY(cache_cbct_moments(c, L, cbct, st));
     DISC_TRY(launch_warp(c, L, ct, disp_inout, L.m, st));

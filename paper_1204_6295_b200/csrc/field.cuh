@@ -82,9 +82,11 @@ __device__ __forceinline__ void force_increment(const float* __restrict__ m, con
 }
 
 // NEXT-3, the paper's "comparison kernel": sum_x |dr(x)| and sum_x |r(x)| (Euclidean norm per
-// voxel, reading A16) of iteration `iter`, per-thread fp32 norms accumulated in fp64; the last block to finish forms
-// l = sum|dr| / sum|r| (+inf while the field is zero), files it in the 16-slot history and, from iteration 10 on,
-// sets stop_iter = iter when l(iter-10) - l(iter) <= stop_eps.  Kernels of later iterations then fall through.
+// voxel, reading A16) of iteration `iter`, per-thread fp32 norms accumulated in fp64.  Every block writes its two
+// partial sums to its own slot; the last block to finish adds them IN BLOCK ORDER (so l, and with it the iteration the
+// level stops at, is the same from run to run), forms l = sum|dr| / sum|r| (+inf while the field is zero), files it in
+// the 16-slot history and, from iteration 10 on, sets stop_iter = iter when l(iter-10) - l(iter) <= stop_eps.  Kernels
+// of later iterations then fall through.
 template <int MODE>
 __global__ void __launch_bounds__(256)
 k_force_norms(const float* __restrict__ m, const float* __restrict__ s, const float* __restrict__ r, int nx, int ny,
@@ -106,28 +108,32 @@ k_force_norms(const float* __restrict__ m, const float* __restrict__ s, const fl
         b += __shfl_xor_sync(0xffffffffu, b, o);
     }
     __shared__ double sh[2][8];
+    __shared__ bool last;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (lane == 0) { sh[0][warp] = a; sh[1][warp] = b; }
     __syncthreads();
     if (threadIdx.x == 0) {
         double ta = 0.0, tb = 0.0;
         for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { ta += sh[0][w]; tb += sh[1][w]; }
-        atomicAdd(&ctl->sum_dr, ta);
-        atomicAdd(&ctl->sum_r, tb);
+        ctl->partial[2 * blockIdx.x] = ta; ctl->partial[2 * blockIdx.x + 1] = tb;
         __threadfence();
-        if (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1) {
-            const double sdr = atomicAdd(&ctl->sum_dr, 0.0), sr = atomicAdd(&ctl->sum_r, 0.0);
-            const double l = sr > 0.0 ? sdr / sr : (double)INFINITY;
-            ctl->hist[iter & 15] = l;
-            if (iter >= 10 && ctl->hist[(iter - 10) & 15] - l <= (double)stop_eps) ctl->stop_iter = iter;
-            ctl->sum_dr = 0.0; ctl->sum_r = 0.0; ctl->ticket = 0u;
-            __threadfence();
-        }
+        last = atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (last && threadIdx.x == 0) {
+        __threadfence();
+        double sdr = 0.0, sr = 0.0;
+        for (unsigned k = 0; k < gridDim.x; ++k) { sdr += ctl->partial[2 * k]; sr += ctl->partial[2 * k + 1]; }
+        const double l = sr > 0.0 ? sdr / sr : (double)INFINITY;
+        ctl->hist[iter & 15] = l;
+        if (iter >= 10 && ctl->hist[(iter - 10) & 15] - l <= (double)stop_eps) ctl->stop_iter = iter;
+        ctl->ticket = 0u;
+        __threadfence();
     }
 }
 
 static __global__ void k_stop_reset(StopCtl* ctl) {
-    ctl->sum_dr = 0.0; ctl->sum_r = 0.0; ctl->ticket = 0u; ctl->stop_iter = 0x7fffffff;
+    ctl->ticket = 0u; ctl->stop_iter = 0x7fffffff;
 }
 static __global__ void k_stop_record(StopCtl* ctl, int level, int n_iters) {
     ctl->runs[level] = ctl->stop_iter == 0x7fffffff ? n_iters : ctl->stop_iter + 1;

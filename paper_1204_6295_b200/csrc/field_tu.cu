@@ -150,6 +150,7 @@ void launch_force_norms(int force, const float* m, const float* s, const float* 
     const size_t N = (size_t)nx * ny * nz;
     size_t blocks = (N + 255) / 256;
     if (blocks > (size_t)8 * n_sm) blocks = (size_t)8 * n_sm;   // grid-stride: one wave of 8 CTAs per SM
+    if (blocks > (size_t)kStopBlocks) blocks = kStopBlocks;
     if (force == kForceDouble)
         k_force_norms<kForceDouble><<<(unsigned)blocks, 256, 0, st>>>(m, s, r, nx, ny, nz, eps_den, ctl, iter, stop_eps);
     else
