@@ -184,7 +184,7 @@ k_gz_warp_d(const float* __restrict__ rin, float* __restrict__ rout, const float
 // Two adjacent columns per thread (nx even, 8-byte aligned fields): 8-byte loads and stores, packed FFMA2 taps --
 // half the load / store / FMA instructions and half the address arithmetic per voxel.
 template <int K, bool WARP, int LZ>
-__global__ void __launch_bounds__(kGzdThreads)
+__global__ void __launch_bounds__(kGzdThreads, 8)   // 64 registers: eight CTAs per SM keep the gathers' latency covered
 k_gz_warp_d2(const float* __restrict__ rin, float* __restrict__ rout, const float* __restrict__ moving,
              float* __restrict__ mout, int nx, int ny, int nz, GaussTaps gw, IterCtl ctl) {
     if (iter_skipped(ctl)) return;
