@@ -24,6 +24,20 @@ static int pick_chunk(int n, int min_chunk, long long ctas_per_chunk, long long 
     return chunk;
 }
 
+template <int K, int FORCE, int TY>
+static void launch_fg_t4(const DevInfo& di, const float* m, const float* s, const float* rin, float* rout, int nx, int ny,
+                         int nz, float eps_den, const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
+    using C = FgT4Cfg<K, TY>;
+    static bool configured[kMaxDevices] = {};  // the opt-in is per device (idempotent, so a race is harmless)
+    if (!configured[di.dev]) {
+        cudaFuncSetAttribute(k_force_gxy_t4<K, FORCE, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
+        configured[di.dev] = true;
+    }
+    const long long n_tiles = (long long)((nx + C::TX - 1) / C::TX) * ((ny + C::TY - 1) / C::TY) * nz;
+    const int grid = (int)(n_tiles < (long long)C::OCC * di.n_sm ? n_tiles : (long long)C::OCC * di.n_sm);   // persistent: OCC CTAs per SM
+    k_force_gxy_t4<K, FORCE, TY><<<grid, C::NT, C::smem_bytes, st>>>(m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl);
+}
+
 template <int K, int FORCE>
 static void launch_fg(const DevInfo& di, const float* m, const float* s, const float* rin, float* rout, int nx, int ny,
                       int nz, float eps_den, const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
@@ -31,15 +45,12 @@ static void launch_fg(const DevInfo& di, const float* m, const float* s, const f
                         3ull * nx * ny * nz < 0xffffffffull;   // the tile kernel indexes voxels with 32 bits
     const int n_sm = di.n_sm;
     if (vec_ok && di.dev >= 0 && di.dev < kMaxDevices) {
-        using C = FgT4Cfg<K>;
-        static bool configured[kMaxDevices] = {};  // the opt-in is per device (idempotent, so a race is harmless)
-        if (!configured[di.dev]) {
-            cudaFuncSetAttribute(k_force_gxy_t4<K, FORCE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
-            configured[di.dev] = true;
-        }
-        const long long n_tiles = (long long)((nx + C::TX - 1) / C::TX) * ((ny + C::TY - 1) / C::TY) * nz;
-        const int grid = (int)(n_tiles < (long long)C::OCC * n_sm ? n_tiles : (long long)C::OCC * n_sm);   // persistent: OCC CTAs per SM
-        k_force_gxy_t4<K, FORCE><<<grid, C::NT, C::smem_bytes, st>>>(m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl);
+        // 64 x 32 tiles; 64 x 8 where those would leave CTA slots of the device empty (small levels)
+        const long long tiles32 = (long long)((nx + 63) / 64) * ((ny + 31) / 32) * nz;
+        if (tiles32 < (long long)FgT4Cfg<K, 32>::OCC * n_sm)
+            launch_fg_t4<K, FORCE, 8>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
+        else
+            launch_fg_t4<K, FORCE, 32>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
         return;
     }
     const int txb = nx > 64 ? 128 : (nx > 32 ? 64 : 32);
@@ -72,16 +83,22 @@ static void launch_gzd2(const float* rin, float* rout, const float* moving, floa
 
 static inline bool aligned8(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 7u) == 0; }
 
-// A thread owns two adjacent columns (one when nx is odd or a field is not 8-byte aligned) and 4 output slices;
-// measured on B200: with two columns per thread 4 slices beat 8 at every level (more threads in flight; the 2K
-// halo re-reads come from L2).
+// A thread owns two adjacent columns (one when nx is odd or a field is not 8-byte aligned) and LZ output slices.
+// Measured on B200: at the fine levels 4 slices beat 8 (more threads in flight; the 2K halo re-reads come from L2).
+// A small level does not fill the device with 4 slices per thread: LZ is halved while the grid stays below a quarter of
+// the device's thread slots (the 13 / LZ re-reads per output hit L2, and the level is latency-bound anyway).
 template <int K, bool WARP>
-static void launch_gz(const float* rin, float* rout, const float* moving, float* mout, int nx, int ny, int nz,
-                      const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
-    if (nx % 2 == 0 && aligned8(rin) && aligned8(rout) && (!WARP || aligned8(mout)))
-        launch_gzd2<K, WARP, 4>(rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
-    else
+static void launch_gz(const DevInfo& di, const float* rin, float* rout, const float* moving, float* mout, int nx, int ny,
+                      int nz, const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
+    const long long want = 512LL * di.n_sm;
+    if (nx % 2 == 0 && aligned8(rin) && aligned8(rout) && (!WARP || aligned8(mout))) {
+        const long long cols = (long long)nx * ny / 2;
+        if (cols * ((nz + 3) / 4) >= want) launch_gzd2<K, WARP, 4>(rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
+        else if (cols * ((nz + 1) / 2) >= want) launch_gzd2<K, WARP, 2>(rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
+        else launch_gzd2<K, WARP, 1>(rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
+    } else {
         launch_gzd<K, WARP, 4>(rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
+    }
 }
 
 // one Gaussian radius: launches if K lies in this unit's range (the discarded branch is never instantiated)
@@ -99,11 +116,11 @@ static bool case_fg(const DevInfo& di, int force, const float* m, const float* s
 }
 
 template <int K>
-static bool case_gz(bool warp, const float* rin, float* rout, const float* moving, float* mout, int nx, int ny, int nz,
+static bool case_gz(const DevInfo& di, bool warp, const float* rin, float* rout, const float* moving, float* mout, int nx, int ny, int nz,
                     const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
     if constexpr (K >= DISC_K_LO && K <= DISC_K_HI) {
-        if (warp) launch_gz<K, true>(rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
-        else launch_gz<K, false>(rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
+        if (warp) launch_gz<K, true>(di, rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
+        else launch_gz<K, false>(di, rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
         return true;
     } else {
         return false;
@@ -127,10 +144,9 @@ bool DISC_CAT(launch_force_gxy_tu, DISC_TU)(const DevInfo& di, int K, int force,
 bool DISC_CAT(launch_gz_warp_tu, DISC_TU)(const DevInfo& di, int K, bool warp, const float* rin, float* rout,
                                           const float* moving, float* mout, int nx, int ny, int nz,
                                           const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
-    (void)di;
     switch (K) {
 #define DISC_CASE(k) \
-    case k: return case_gz<k>(warp, rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
+    case k: return case_gz<k>(di, warp, rin, rout, moving, mout, nx, ny, nz, taps, ctl, st);
         DISC_FOR_K(DISC_CASE)
 #undef DISC_CASE
     }

@@ -269,18 +269,15 @@ k_gz_warp_d2(const float* __restrict__ rin, float* __restrict__ rout, const floa
 #ifndef DISC_FG_LX
 #define DISC_FG_LX 8
 #endif
-#ifndef DISC_FG_TY
-#define DISC_FG_TY 32
-#endif
 #ifndef DISC_FG_NT
 #define DISC_FG_NT 256
 #endif
 #ifndef DISC_FG_OCC
 #define DISC_FG_OCC 2
 #endif
-template <int K>
+template <int K, int TY_>
 struct FgT4Cfg {
-    static constexpr int TX = 64, TY = DISC_FG_TY, NT = DISC_FG_NT, OCC = DISC_FG_OCC, LX = DISC_FG_LX, LY = 8;
+    static constexpr int TX = 64, TY = TY_, NT = DISC_FG_NT, OCC = DISC_FG_OCC, LX = DISC_FG_LX, LY = 8;
     static constexpr int W = 2 * K + 1;
     static constexpr int KA = (K + 3) / 4 * 4, OFF = KA - K;
     static constexpr int PXA = TX + 2 * KA, PY = TY + 2 * K, NG = PXA / 4;
@@ -371,16 +368,18 @@ struct FgGroup {
     }
 };
 
+// The tile is 64 x TY_: 32 rows at the fine levels; 8 rows where a level has fewer 64 x 32 tiles than the device has
+// CTA slots (64 x 64 x 32: 64 tiles) -- four times the CTAs, each with a quarter of the serial work per phase.
 // PERSISTENT: the grid is two CTAs per SM; a CTA walks tiles t = blockIdx.x, += gridDim.x (x fastest, so the CTAs
 // running at the same time work on neighbouring tiles and share their halos in L2).  Phase 3 of tile t-1 and
 // phase 1 of tile t share one barrier interval -- the y pass (pure FMA work out of shared memory) runs on some
 // warps while others wait for phase 1's global loads.
-template <int K, int FORCE>
-__global__ void __launch_bounds__(FgT4Cfg<K>::NT, FgT4Cfg<K>::OCC)
+template <int K, int FORCE, int TY_>
+__global__ void __launch_bounds__(FgT4Cfg<K, TY_>::NT, FgT4Cfg<K, TY_>::OCC)
 k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const float* __restrict__ rin,
                float* __restrict__ rout, int nx, int ny, int nz, float eps_den, GaussTaps gw, IterCtl ctl) {
     if (iter_skipped(ctl)) return;
-    using C = FgT4Cfg<K>;
+    using C = FgT4Cfg<K, TY_>;
     constexpr int W = C::W, TX = C::TX, TY = C::TY, NT = C::NT, LX = C::LX, LY = C::LY, PY = C::PY, NG = C::NG;
     constexpr int UP = C::UP, XP = C::XP, KA = C::KA, OFF = C::OFF, NV = C::NV;
     extern __shared__ __align__(16) float smem_f[];
@@ -400,16 +399,20 @@ k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const f
         const int z = t / (ntx * nty), txy = t - z * (ntx * nty);
         const int y0 = (txy / ntx) * TY, x0 = (txy - (txy / ntx) * ntx) * TX;
 
-        // ---- phase 1 of tile t: updated field at the tile + halo, four x-adjacent points at a time
+        // ---- phase 1 of tile t: updated field at the tile + halo, four x-adjacent points at a time.  Two groups per
+        // thread and round, both groups' loads issued before either is evaluated: phase 1 is bound by the latency of
+        // its loads (profiles/r02a: 55 % of the kernel's stall samples on 36 % of its instructions), and twice the
+        // loads in flight halves the number of exposed round trips per tile.
         if (have) {
-            for (int p = tid; p < PY * NG; p += NT) {
-                const int r = p / NG, g = p - r * NG;
+            auto issue = [&](FgGroup<FORCE>& G, int p, int& r, int& g, int& gx) {
+                r = p / NG; g = p - r * NG;
                 const int gy = clampi(y0 - K + r, 0, ny - 1);
-                const int gx = x0 - KA + 4 * g;
-                // a group wholly outside the volume is the replicate border: the edge group's outermost value
-                FgGroup<FORCE> G;
+                gx = x0 - KA + 4 * g;
                 G.load(m, s, rin, nx, ny, nz, (unsigned)plane, (unsigned)N, clampi(gx, 0, nx - 4), gy, z);
+            };
+            auto retire = [&](FgGroup<FORCE>& G, int r, int g, int gx) {
                 G.finish(eps_den);
+                // a group wholly outside the volume is the replicate border: the edge group's outermost value
                 if (gx < 0 || gx >= nx) {   // only in the tiles at the volume's x border
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
@@ -419,6 +422,15 @@ k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const f
                 }
 #pragma unroll
                 for (int c = 0; c < 3; ++c) *reinterpret_cast<float4*>(U + (c * PY + r) * UP + 4 * g) = G.u[c];
+            };
+            for (int p = tid; p < PY * NG; p += 2 * NT) {
+                FgGroup<FORCE> G0, G1;
+                int r0, g0, gx0, r1 = 0, g1 = 0, gx1 = 0;
+                const bool two = p + NT < PY * NG;
+                issue(G0, p, r0, g0, gx0);
+                if (two) issue(G1, p + NT, r1, g1, gx1);
+                retire(G0, r0, g0, gx0);
+                if (two) retire(G1, r1, g1, gx1);
             }
         }
         // ---- phase 3 of tile t-1: y pass, lanes <-> column groups

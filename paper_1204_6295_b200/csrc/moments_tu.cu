@@ -2,6 +2,7 @@
 // (-DDISC_TU=n -DDISC_R_LO=a -DDISC_R_HI=b) so the instances compile in parallel.
 #include "launch.h"
 #include "moments.cuh"
+#include "moments_blk.cuh"
 #include "moments_v3.cuh"
 
 #define DISC_CAT2(a, b) a##b
@@ -90,6 +91,54 @@ static bool launch_r_v3(const DevInfo& di, int rz, int mode, const float* vol, c
     return true;
 }
 
+// Small volumes (the coarse pyramid levels): the block kernel of moments_blk.cuh.  A block is 32 x by x bz outputs;
+// (by, bz) is the largest block whose raw tile + pair buffer fit shared memory, and the kernel is taken only while
+// the whole grid is at most two waves of one CTA per SM -- beyond that the marching kernel's O(1) halo wins.
+template <int R>
+static bool launch_r_blk(const DevInfo& di, int rz, int mode, const float* vol, const float* aux, float* out0,
+                         float* out1, int nx, int ny, int nz, float eps_var, IterCtl ctl, cudaStream_t st) {
+    using C = MomBlkCfg<R>;
+    if (2 * rz + 1 > kMaxWz) return false;
+    constexpr size_t kSmemMax = 216 * 1024;
+    static const int cand[][2] = {{8, 4}, {8, 2}, {4, 4}, {4, 2}};
+    int by = 0, bz = 0;
+    for (const auto& c : cand)
+        if (C::smem_bytes(c[0] + 2 * R, c[1] + 2 * rz) <= kSmemMax) { by = c[0]; bz = c[1]; break; }
+    if (by * bz < 16) return false;
+    const long long ctas = (long long)((nx + C::TX - 1) / C::TX) * ((ny + by - 1) / by) * ((nz + bz - 1) / bz);
+    if (ctas > 2LL * di.n_sm) return false;
+    const int py = by + 2 * R, pz = bz + 2 * rz;
+    if (py > 256 || pz > 256) return false;
+    EncodeTiledFn enc = encode_tiled();
+    if (!enc) return false;
+    CUtensorMap tmap;
+    const cuuint64_t gdim[3] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz};
+    const cuuint64_t gstr[2] = {(cuuint64_t)nx * 4, (cuuint64_t)nx * ny * 4};
+    const cuuint32_t box[3] = {(cuuint32_t)C::PXB, (cuuint32_t)py, (cuuint32_t)pz};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(vol), gdim, gstr, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return false;
+    const float* pv = mode == kModeCorrect ? aux : vol;
+    dim3 grid((nx + C::TX - 1) / C::TX, (ny + by - 1) / by, (nz + bz - 1) / bz);
+    const size_t smem = C::smem_bytes(py, pz);
+    static bool configured[3][kMaxDevices] = {};
+#define DISC_LAUNCH_MODE(M)                                                                                              \
+    {                                                                                                                    \
+        if (!configured[M][di.dev]) {   /* the opt-in is per device */                                                   \
+            cudaFuncSetAttribute(k_moments_blk<R, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);       \
+            configured[M][di.dev] = true;                                                                                \
+        }                                                                                                                \
+        k_moments_blk<R, M><<<grid, C::NT, smem, st>>>(tmap, pv, out0, out1, nx, ny, nz, rz, by, bz, eps_var, ctl);      \
+    }
+    if (mode == kModeMoments) DISC_LAUNCH_MODE(kModeMoments)
+    else if (mode == kModeZscore) DISC_LAUNCH_MODE(kModeZscore)
+    else DISC_LAUNCH_MODE(kModeCorrect)
+#undef DISC_LAUNCH_MODE
+    return true;
+}
+
 // the TMA kernel with the tile height the z window allows: 32 rows while the ring of 2 rz + 1 slots fits tensor
 // memory, 16 rows beyond (possible only when the tile + halo still has 32 rows, R >= 8)
 template <int R>
@@ -111,7 +160,8 @@ static bool launch_r(const DevInfo& di, int rz, int mode, const float* vol, cons
     if (di.dev < 0 || di.dev >= kMaxDevices) return false;
     // TMA path: rows must be 16-byte multiples and the base 16-byte aligned (tensor-map requirements)
     if (nx % 4 == 0 && (reinterpret_cast<uintptr_t>(vol) & 15u) == 0 &&
-        launch_r_tma<R>(di, rz, mode, vol, aux, out0, out1, nx, ny, nz, eps_var, ctl, st))
+        (launch_r_blk<R>(di, rz, mode, vol, aux, out0, out1, nx, ny, nz, eps_var, ctl, st) ||
+         launch_r_tma<R>(di, rz, mode, vol, aux, out0, out1, nx, ny, nz, eps_var, ctl, st)))
         return true;
     if constexpr (R <= 10) {
         if (rz == R) {   // plain-load sliding-window kernel: cubic patches, any nx
