@@ -270,24 +270,35 @@ k_gz_warp_d2(const float* __restrict__ rin, float* __restrict__ rout, const floa
 #define DISC_FG_LX 8
 #endif
 #ifndef DISC_FG_NT
-#define DISC_FG_NT 256
+#define DISC_FG_NT 224
 #endif
 #ifndef DISC_FG_OCC
 #define DISC_FG_OCC 2
 #endif
+// Shared-memory layouts (tile 64 x TY, halo K in y, KA = K rounded up to 4 in x; PY = TY + 2K rows, always even):
+//   U  updated field at the tile + halo, ROW-PAIR INTERLEAVED: U[c][rp][x][2] holds rows 2rp and 2rp+1 of column x
+//      side by side, so that the x pass finds (row 2rp, row 2rp+1) of every column in one aligned 64-bit register
+//      pair and runs as packed FFMA2 over two rows at once -- whatever the tap, the pair is aligned (pairs ALONG x
+//      would be misaligned for every odd tap);
+//   X  x-smoothed field, plain rows grouped in pairs: row R at (R >> 1) * XPP + (R & 1) * XP, XPP an odd number of
+//      16-byte chunks (lanes <-> row pairs store conflict free), read by the y pass with lanes <-> column groups.
 template <int K, int TY_>
 struct FgT4Cfg {
     static constexpr int TX = 64, TY = TY_, NT = DISC_FG_NT, OCC = DISC_FG_OCC, LX = DISC_FG_LX, LY = 8;
     static constexpr int W = 2 * K + 1;
     static constexpr int KA = (K + 3) / 4 * 4, OFF = KA - K;
-    static constexpr int PXA = TX + 2 * KA, PY = TY + 2 * K, NG = PXA / 4;
-    static constexpr int UP = ((PXA / 4) | 1) * 4;               // U row pitch: odd number of 16-byte chunks
-    static constexpr int XP = TX + 4;                            // X row pitch: 17 chunks (odd)
-    static constexpr int NV = (OFF + LX + 2 * K + 3) / 4;        // 16-byte chunks of one x-pass run
-    static constexpr int P2_TASKS = 3 * PY * (TX / LX);
+    static constexpr int PXA = TX + 2 * KA, PY = TY + 2 * K, NG = PXA / 4, NRP = PY / 2;
+    static constexpr int UPP = ((2 * PXA / 4) | 1) * 4;          // U row-pair pitch in floats: odd number of 16-byte chunks
+    static constexpr int XP = TX + 4;                            // X row pitch
+    static constexpr int XPP = ((2 * XP / 4) | 1) * 4;           // X row-pair pitch: odd number of 16-byte chunks
+    static constexpr int O4 = (2 * OFF) / 4, O2 = (2 * OFF) % 4; // first chunk / float of an x-pass run inside its segment
+    static constexpr int NV = (O2 + 2 * (LX + 2 * K) + 3) / 4;   // 16-byte chunks of one x-pass run (two rows)
+    static constexpr int P1_TASKS = NRP * NG;
+    static constexpr int P2_TASKS = 3 * NRP * (TX / LX);
     static constexpr int P3_TASKS = 3 * (TX / 4) * (TY / LY);
-    static constexpr size_t smem_bytes = sizeof(float) * 3 * PY * (UP + XP);
-    static_assert((TX - LX) + 4 * NV <= UP, "x-pass run must stay inside the U row");
+    static constexpr size_t smem_bytes = sizeof(float) * 3 * NRP * (UPP + XPP);
+    static_assert(PY % 2 == 0 && TY % LY == 0 && TX % LX == 0 && LX % 4 == 0, "tile shape");
+    static_assert(2 * (TX - LX) + 4 * (O4 + NV) <= UPP, "x-pass run must stay inside the U row pair");
 };
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
@@ -296,6 +307,23 @@ __device__ __forceinline__ float rcp_approx(float x) {
     float r;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
+}
+
+// packed fp32x2 add / subtract / multiply (Blackwell): both halves round exactly like the scalar instruction
+__device__ __forceinline__ float2 fadd2(float2 a, float2 b) {
+    unsigned long long ra = *reinterpret_cast<unsigned long long*>(&a), rb = *reinterpret_cast<unsigned long long*>(&b), rd;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(rd) : "l"(ra), "l"(rb));
+    return *reinterpret_cast<float2*>(&rd);
+}
+__device__ __forceinline__ float2 fsub2(float2 a, float2 b) {
+    unsigned long long ra = *reinterpret_cast<unsigned long long*>(&a), rb = *reinterpret_cast<unsigned long long*>(&b), rd;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(rd) : "l"(ra), "l"(rb));
+    return *reinterpret_cast<float2*>(&rd);
+}
+__device__ __forceinline__ float2 fmul2(float2 a, float2 b) {
+    unsigned long long ra = *reinterpret_cast<unsigned long long*>(&a), rb = *reinterpret_cast<unsigned long long*>(&b), rd;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(rd) : "l"(ra), "l"(rb));
+    return *reinterpret_cast<float2*>(&rd);
 }
 
 // updated field of one group of four x-adjacent points (gx % 4 == 0), loads first, arithmetic after.
@@ -310,60 +338,63 @@ struct FgGroup {
     float sl, sr;
     float4 myp, mym, mzp, mzm;   // double force only: the moving image's neighbours
     float ml, mr;
+    // The group's own row and its z neighbours; the y neighbours (sym, syp, [mym, myp]) and the x neighbours
+    // (sl, sr, [ml, mr]) are filled in by the caller, which shares them between the two rows of a pair and between
+    // the lanes of a warp.
     __device__ __forceinline__ void load(const float* __restrict__ m, const float* __restrict__ s,
-                                         const float* __restrict__ rin, int nx, int ny, int nz, unsigned plane, unsigned N,
-                                         int gx, int gy, int z) {
-        const unsigned i = (unsigned)z * plane + (unsigned)gy * (unsigned)nx + (unsigned)gx;
+                                         const float* __restrict__ rin, int nz, unsigned plane, unsigned N, unsigned i,
+                                         int z) {
 #pragma unroll
         for (int c = 0; c < 3; ++c) u[c] = ldg4(rin + (i + (unsigned)c * N));
         if (FORCE) {
-            const unsigned il = i - (gx > 0 ? 1u : 0u), ir = i + 3u + (gx + 4 < nx ? 1u : 0u);
-            const unsigned iyp = i + (gy < ny - 1 ? (unsigned)nx : 0u), iym = i - (gy > 0 ? (unsigned)nx : 0u);
             const unsigned izp = i + (z < nz - 1 ? plane : 0u), izm = i - (z > 0 ? plane : 0u);
             sc = ldg4(s + i); mm = ldg4(m + i);
-            sl = __ldg(s + il); sr = __ldg(s + ir);
-            syp = ldg4(s + iyp); sym = ldg4(s + iym);
             szp = ldg4(s + izp); szm = ldg4(s + izm);
-            if (FORCE == kForceDouble) {
-                ml = __ldg(m + il); mr = __ldg(m + ir);
-                myp = ldg4(m + iyp); mym = ldg4(m + iym);
-                mzp = ldg4(m + izp); mzm = ldg4(m + izm);
-            }
+            if (FORCE == kForceDouble) { mzp = ldg4(m + izp); mzm = ldg4(m + izm); }
         }
     }
+    // Two points at a time (x-adjacent halves of the 16-byte loads) with packed fp32x2 arithmetic: the same operations
+    // in the same order as the scalar form, so every half rounds identically; only the x differences, whose operands
+    // straddle the halves, and the two reciprocals are scalar.
     __device__ __forceinline__ void finish(float eps_den) {
         if (FORCE) {
-            const float ce[6] = {sl, sc.x, sc.y, sc.z, sc.w, sr};
-            const float me[4] = {mm.x, mm.y, mm.z, mm.w};
-            const float yp[4] = {syp.x, syp.y, syp.z, syp.w}, ym[4] = {sym.x, sym.y, sym.z, sym.w};
-            const float zp[4] = {szp.x, szp.y, szp.z, szp.w}, zm[4] = {szm.x, szm.y, szm.z, szm.w};
-            float ux[4] = {u[0].x, u[0].y, u[0].z, u[0].w}, uy[4] = {u[1].x, u[1].y, u[1].z, u[1].w};
-            float uz[4] = {u[2].x, u[2].y, u[2].z, u[2].w};
-            const float he[6] = {ml, mm.x, mm.y, mm.z, mm.w, mr};
-            const float hyp[4] = {myp.x, myp.y, myp.z, myp.w}, hym[4] = {mym.x, mym.y, mym.z, mym.w};
-            const float hzp[4] = {mzp.x, mzp.y, mzp.z, mzp.w}, hzm[4] = {mzm.x, mzm.y, mzm.z, mzm.w};
-            const float eps4 = 4.f * eps_den;
+            const float2 eps4 = make_float2(4.f * eps_den, 4.f * eps_den);
+            const float2 scp[2] = {make_float2(sc.x, sc.y), make_float2(sc.z, sc.w)};
+            const float2 mmp[2] = {make_float2(mm.x, mm.y), make_float2(mm.z, mm.w)};
+            const float2 ypp[2] = {make_float2(syp.x, syp.y), make_float2(syp.z, syp.w)};
+            const float2 ymp[2] = {make_float2(sym.x, sym.y), make_float2(sym.z, sym.w)};
+            const float2 zpp[2] = {make_float2(szp.x, szp.y), make_float2(szp.z, szp.w)};
+            const float2 zmp[2] = {make_float2(szm.x, szm.y), make_float2(szm.z, szm.w)};
+            const float2 Dxp[2] = {make_float2(sc.y - sl, sc.z - sc.x), make_float2(sc.w - sc.y, sr - sc.z)};
+            float2 up[3][2] = {{make_float2(u[0].x, u[0].y), make_float2(u[0].z, u[0].w)},
+                               {make_float2(u[1].x, u[1].y), make_float2(u[1].z, u[1].w)},
+                               {make_float2(u[2].x, u[2].y), make_float2(u[2].z, u[2].w)}};
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const float Dx = ce[e + 2] - ce[e], Dy = yp[e] - ym[e], Dz = zp[e] - zm[e];
-                const float d = ce[e + 1] - me[e];
-                const float t = d + d;
-                const float tt = fmaf(t, t, eps4);
-                const float q = t * rcp_approx(fmaf(Dx, Dx, fmaf(Dy, Dy, fmaf(Dz, Dz, tt))));
-                ux[e] = fmaf(q, Dx, ux[e]);
-                uy[e] = fmaf(q, Dy, uy[e]);
-                uz[e] = fmaf(q, Dz, uz[e]);
+            for (int h = 0; h < 2; ++h) {
+                const float2 Dx = Dxp[h], Dy = fsub2(ypp[h], ymp[h]), Dz = fsub2(zpp[h], zmp[h]);
+                const float2 d = fsub2(scp[h], mmp[h]);
+                const float2 t = fadd2(d, d);
+                const float2 tt = ffma2(t, t, eps4);
+                const float2 den = ffma2(Dx, Dx, ffma2(Dy, Dy, ffma2(Dz, Dz, tt)));
+                const float2 q = fmul2(t, make_float2(rcp_approx(den.x), rcp_approx(den.y)));
+                up[0][h] = ffma2(q, Dx, up[0][h]);
+                up[1][h] = ffma2(q, Dy, up[1][h]);
+                up[2][h] = ffma2(q, Dz, up[2][h]);
                 if (FORCE == kForceDouble) {
-                    const float Hx = he[e + 2] - he[e], Hy = hyp[e] - hym[e], Hz = hzp[e] - hzm[e];
-                    const float p = t * rcp_approx(fmaf(Hx, Hx, fmaf(Hy, Hy, fmaf(Hz, Hz, tt))));
-                    ux[e] = fmaf(p, Hx, ux[e]);
-                    uy[e] = fmaf(p, Hy, uy[e]);
-                    uz[e] = fmaf(p, Hz, uz[e]);
+                    const float2 Hx = h == 0 ? make_float2(mm.y - ml, mm.z - mm.x) : make_float2(mm.w - mm.y, mr - mm.z);
+                    const float2 Hy = h == 0 ? fsub2(make_float2(myp.x, myp.y), make_float2(mym.x, mym.y))
+                                             : fsub2(make_float2(myp.z, myp.w), make_float2(mym.z, mym.w));
+                    const float2 Hz = h == 0 ? fsub2(make_float2(mzp.x, mzp.y), make_float2(mzm.x, mzm.y))
+                                             : fsub2(make_float2(mzp.z, mzp.w), make_float2(mzm.z, mzm.w));
+                    const float2 dh = ffma2(Hx, Hx, ffma2(Hy, Hy, ffma2(Hz, Hz, tt)));
+                    const float2 p = fmul2(t, make_float2(rcp_approx(dh.x), rcp_approx(dh.y)));
+                    up[0][h] = ffma2(p, Hx, up[0][h]);
+                    up[1][h] = ffma2(p, Hy, up[1][h]);
+                    up[2][h] = ffma2(p, Hz, up[2][h]);
                 }
             }
-            u[0] = make_float4(ux[0], ux[1], ux[2], ux[3]);
-            u[1] = make_float4(uy[0], uy[1], uy[2], uy[3]);
-            u[2] = make_float4(uz[0], uz[1], uz[2], uz[3]);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) u[c] = make_float4(up[c][0].x, up[c][0].y, up[c][1].x, up[c][1].y);
         }
     }
 };
@@ -380,11 +411,11 @@ k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const f
                float* __restrict__ rout, int nx, int ny, int nz, float eps_den, GaussTaps gw, IterCtl ctl) {
     if (iter_skipped(ctl)) return;
     using C = FgT4Cfg<K, TY_>;
-    constexpr int W = C::W, TX = C::TX, TY = C::TY, NT = C::NT, LX = C::LX, LY = C::LY, PY = C::PY, NG = C::NG;
-    constexpr int UP = C::UP, XP = C::XP, KA = C::KA, OFF = C::OFF, NV = C::NV;
+    constexpr int W = C::W, TX = C::TX, TY = C::TY, NT = C::NT, LX = C::LX, LY = C::LY, NG = C::NG, NRP = C::NRP;
+    constexpr int UPP = C::UPP, XP = C::XP, XPP = C::XPP, KA = C::KA, NV = C::NV;
     extern __shared__ __align__(16) float smem_f[];
-    float* U = smem_f;                       // [3][PY][UP]
-    float* X = smem_f + 3 * PY * UP;         // [3][PY][XP]
+    float* U = smem_f;                        // [3][NRP][UPP]
+    float* X = smem_f + 3 * NRP * UPP;        // [3][NRP][XPP]
 
     const int tid = threadIdx.x;
     const size_t plane = (size_t)nx * ny;
@@ -399,76 +430,99 @@ k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const f
         const int z = t / (ntx * nty), txy = t - z * (ntx * nty);
         const int y0 = (txy / ntx) * TY, x0 = (txy - (txy / ntx) * ntx) * TX;
 
-        // ---- phase 1 of tile t: updated field at the tile + halo, four x-adjacent points at a time.  Two groups per
-        // thread and round, both groups' loads issued before either is evaluated: phase 1 is bound by the latency of
-        // its loads (profiles/r02a: 55 % of the kernel's stall samples on 36 % of its instructions), and twice the
-        // loads in flight halves the number of exposed round trips per tile.
-        if (have) {
-            auto issue = [&](FgGroup<FORCE>& G, int p, int& r, int& g, int& gx) {
-                r = p / NG; g = p - r * NG;
-                const int gy = clampi(y0 - K + r, 0, ny - 1);
-                gx = x0 - KA + 4 * g;
-                G.load(m, s, rin, nx, ny, nz, (unsigned)plane, (unsigned)N, clampi(gx, 0, nx - 4), gy, z);
-            };
-            auto retire = [&](FgGroup<FORCE>& G, int r, int g, int gx) {
-                G.finish(eps_den);
-                // a group wholly outside the volume is the replicate border: the edge group's outermost value
-                if (gx < 0 || gx >= nx) {   // only in the tiles at the volume's x border
+        // ================= first interval: phase 1 of tile t, phase 3 of tile t-1
+        {
+            if (have) {
+                // ---- phase 1: updated field at the tile + halo.  A task is a ROW PAIR of one group of four x-adjacent
+                // points, all loads issued before either row is evaluated; rows 2rp and 2rp+1 are each other's y
+                // neighbours (4 row loads of s' instead of 6).
+                for (int p = tid; p < C::P1_TASKS; p += NT) {
+                    const int rp = p / NG, g = p - rp * NG;
+                    const int gy0 = clampi(y0 - K + 2 * rp, 0, ny - 1), gy1 = clampi(y0 - K + 2 * rp + 1, 0, ny - 1);
+                    const int gx = x0 - KA + 4 * g;
+                    const int gxc = clampi(gx, 0, nx - 4);
+                    const unsigned i0 = (unsigned)z * (unsigned)plane + (unsigned)gy0 * (unsigned)nx + (unsigned)gxc;
+                    const unsigned i1 = (unsigned)z * (unsigned)plane + (unsigned)gy1 * (unsigned)nx + (unsigned)gxc;
+                    FgGroup<FORCE> G0, G1;
+                    G0.load(m, s, rin, nz, (unsigned)plane, (unsigned)N, i0, z);
+                    G1.load(m, s, rin, nz, (unsigned)plane, (unsigned)N, i1, z);
+                    if (FORCE) {
+                        const unsigned dl = gxc > 0 ? 1u : 0u, dr = 3u + (gxc + 4 < nx ? 1u : 0u);
+                        const unsigned im = i0 - (gy0 > 0 ? (unsigned)nx : 0u), ip = i1 + (gy1 < ny - 1 ? (unsigned)nx : 0u);
+                        const float4 sym0 = ldg4(s + im), syp1 = ldg4(s + ip);
+                        G0.sl = __ldg(s + (i0 - dl)); G1.sl = __ldg(s + (i1 - dl));
+                        G0.sr = __ldg(s + (i0 + dr)); G1.sr = __ldg(s + (i1 + dr));
+                        // rows gy0, gy1 are adjacent, or both clamped to the same border row (then the two groups are equal)
+                        const bool adj = gy1 != gy0;
+                        G0.sym = sym0; G1.syp = syp1;
+                        G0.syp = adj ? G1.sc : syp1;
+                        G1.sym = adj ? G0.sc : sym0;
+                        if (FORCE == kForceDouble) {
+                            const float4 mym0 = ldg4(m + im), myp1 = ldg4(m + ip);
+                            G0.ml = __ldg(m + (i0 - dl)); G1.ml = __ldg(m + (i1 - dl));
+                            G0.mr = __ldg(m + (i0 + dr)); G1.mr = __ldg(m + (i1 + dr));
+                            G0.mym = mym0; G1.myp = myp1;
+                            G0.myp = adj ? G1.mm : myp1;
+                            G1.mym = adj ? G0.mm : mym0;
+                        }
+                    }
+                    G0.finish(eps_den);
+                    G1.finish(eps_den);
+                    // a group wholly outside the volume is the replicate border: the edge group's outermost value
+                    if (gx < 0 || gx >= nx) {   // only in the tiles at the volume's x border
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            const float e0 = gx < 0 ? G0.u[c].x : G0.u[c].w, e1 = gx < 0 ? G1.u[c].x : G1.u[c].w;
+                            G0.u[c] = make_float4(e0, e0, e0, e0);
+                            G1.u[c] = make_float4(e1, e1, e1, e1);
+                        }
+                    }
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
-                        const float e = gx < 0 ? G.u[c].x : G.u[c].w;
-                        G.u[c] = make_float4(e, e, e, e);
+                        float4* up = reinterpret_cast<float4*>(U + (c * NRP + rp) * UPP + 8 * g);
+                        up[0] = make_float4(G0.u[c].x, G1.u[c].x, G0.u[c].y, G1.u[c].y);
+                        up[1] = make_float4(G0.u[c].z, G1.u[c].z, G0.u[c].w, G1.u[c].w);
                     }
                 }
-#pragma unroll
-                for (int c = 0; c < 3; ++c) *reinterpret_cast<float4*>(U + (c * PY + r) * UP + 4 * g) = G.u[c];
-            };
-            for (int p = tid; p < PY * NG; p += 2 * NT) {
-                FgGroup<FORCE> G0, G1;
-                int r0, g0, gx0, r1 = 0, g1 = 0, gx1 = 0;
-                const bool two = p + NT < PY * NG;
-                issue(G0, p, r0, g0, gx0);
-                if (two) issue(G1, p + NT, r1, g1, gx1);
-                retire(G0, r0, g0, gx0);
-                if (two) retire(G1, r1, g1, gx1);
             }
-        }
-        // ---- phase 3 of tile t-1: y pass, lanes <-> column groups
-        if (have_prev) {
-            for (int tk = tid; tk < C::P3_TASKS; tk += NT) {
-                const int cg = tk % (TX / 4), q = tk / (TX / 4), h = q % (TY / LY), cc = q / (TY / LY);
-                const float4* xp = reinterpret_cast<const float4*>(X + (cc * PY + h * LY) * XP + cg * 4);
-                float2 a0[LY], a1[LY];
+            if (have_prev) {
+                // ---- phase 3 of tile t-1: y pass, lanes <-> column groups
+                for (int tk = tid; tk < C::P3_TASKS; tk += NT) {
+                    const int cg = tk % (TX / 4), q = tk / (TX / 4), h = q % (TY / LY), cc = q / (TY / LY);
+                    const float* xb = X + cc * NRP * XPP + cg * 4;
+                    float2 a0[LY], a1[LY];
 #pragma unroll
-                for (int j = 0; j < LY; ++j) { a0[j] = make_float2(0.f, 0.f); a1[j] = make_float2(0.f, 0.f); }
+                    for (int j = 0; j < LY; ++j) { a0[j] = make_float2(0.f, 0.f); a1[j] = make_float2(0.f, 0.f); }
 #pragma unroll
-                for (int i = 0; i < LY + 2 * K; ++i) {
-                    const float4 f = xp[i * (XP / 4)];
-                    const float2 lo = make_float2(f.x, f.y), hi = make_float2(f.z, f.w);
-#pragma unroll
-                    for (int j = 0; j < LY; ++j) {
-                        const int k = i - j;          // input row i contributes to output row j with tap k
-                        if (k >= 0 && k < W) {
-                            const float2 w2 = make_float2(gw.w[k], gw.w[k]);
-                            a0[j] = ffma2(w2, lo, a0[j]);
-                            a1[j] = ffma2(w2, hi, a1[j]);
-                        }
-                    }
-                }
-                const int gx = px0 + cg * 4;
-                if (gx < nx) {
-                    float* op = rout + cc * N + ((size_t)pz * ny + (py0 + h * LY)) * nx + gx;
-                    if (py0 + h * LY + LY <= ny) {   // whole run inside the volume: no per-row test
+                    for (int i = 0; i < LY + 2 * K; ++i) {
+                        const int row = h * LY + i;       // LY is even: the parity of the row is the parity of i
+                        const float4 f = *reinterpret_cast<const float4*>(xb + (row >> 1) * XPP + (i & 1) * XP);
+                        const float2 lo = make_float2(f.x, f.y), hi = make_float2(f.z, f.w);
 #pragma unroll
                         for (int j = 0; j < LY; ++j) {
-                            *reinterpret_cast<float4*>(op) = make_float4(a0[j].x, a0[j].y, a1[j].x, a1[j].y);
-                            op += nx;
+                            const int k = i - j;          // input row i contributes to output row j with tap k
+                            if (k >= 0 && k < W) {
+                                const float2 w2 = make_float2(gw.w[k], gw.w[k]);
+                                a0[j] = ffma2(w2, lo, a0[j]);
+                                a1[j] = ffma2(w2, hi, a1[j]);
+                            }
                         }
-                    } else {
+                    }
+                    const int gx = px0 + cg * 4;
+                    if (gx < nx) {
+                        float* op = rout + cc * N + ((size_t)pz * ny + (py0 + h * LY)) * nx + gx;
+                        if (py0 + h * LY + LY <= ny) {   // whole run inside the volume: no per-row test
 #pragma unroll
-                        for (int j = 0; j < LY; ++j)
-                            if (py0 + h * LY + j < ny)
-                                *reinterpret_cast<float4*>(op + (size_t)j * nx) = make_float4(a0[j].x, a0[j].y, a1[j].x, a1[j].y);
+                            for (int j = 0; j < LY; ++j) {
+                                *reinterpret_cast<float4*>(op) = make_float4(a0[j].x, a0[j].y, a1[j].x, a1[j].y);
+                                op += nx;
+                            }
+                        } else {
+#pragma unroll
+                            for (int j = 0; j < LY; ++j)
+                                if (py0 + h * LY + j < ny)
+                                    *reinterpret_cast<float4*>(op + (size_t)j * nx) = make_float4(a0[j].x, a0[j].y, a1[j].x, a1[j].y);
+                        }
                     }
                 }
             }
@@ -476,27 +530,34 @@ k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const f
         if (!have) break;
         __syncthreads();
 
-        // ---- phase 2 of tile t: x pass, lanes <-> rows; output x0 + g*LX + j reads U columns OFF + g*LX + j + k
-        for (int tk = tid; tk < C::P2_TASKS; tk += NT) {
-            const int r = tk % PY, q = tk / PY, g = q % (TX / LX), cc = q / (TX / LX);
-            const float4* up = reinterpret_cast<const float4*>(U + (cc * PY + r) * UP + g * LX);
-            float v[4 * NV];
+        // ================= second interval: phase 2 of tile t, x pass over two rows at once, lanes <-> row pairs.
+        // Output column x0 + g*LX + j of both rows reads the pairs of columns OFF + g*LX + j + k: one packed FFMA2 per
+        // tap and output pair.
+        {
+            for (int tk = tid; tk < C::P2_TASKS; tk += NT) {
+                const int rp = tk % NRP, q = tk / NRP, g = q % (TX / LX), cc = q / (TX / LX);
+                const float4* up = reinterpret_cast<const float4*>(U + (cc * NRP + rp) * UPP + 2 * g * LX) + C::O4;
+                float2 v[2 * NV];
 #pragma unroll
-            for (int i = 0; i < NV; ++i) {
-                const float4 f = up[i];
-                v[4 * i] = f.x; v[4 * i + 1] = f.y; v[4 * i + 2] = f.z; v[4 * i + 3] = f.w;
+                for (int i = 0; i < NV; ++i) {
+                    const float4 f = up[i];
+                    v[2 * i] = make_float2(f.x, f.y); v[2 * i + 1] = make_float2(f.z, f.w);
+                }
+                float2 o[LX];
+#pragma unroll
+                for (int j = 0; j < LX; ++j) {
+                    float2 acc = make_float2(0.f, 0.f);
+#pragma unroll
+                    for (int k = 0; k < W; ++k) acc = ffma2(make_float2(gw.w[k], gw.w[k]), v[C::O2 / 2 + j + k], acc);
+                    o[j] = acc;
+                }
+                float* xr = X + (cc * NRP + rp) * XPP + g * LX;
+#pragma unroll
+                for (int q4 = 0; q4 < LX / 4; ++q4) {
+                    *reinterpret_cast<float4*>(xr + 4 * q4) = make_float4(o[4 * q4].x, o[4 * q4 + 1].x, o[4 * q4 + 2].x, o[4 * q4 + 3].x);
+                    *reinterpret_cast<float4*>(xr + XP + 4 * q4) = make_float4(o[4 * q4].y, o[4 * q4 + 1].y, o[4 * q4 + 2].y, o[4 * q4 + 3].y);
+                }
             }
-            float o[LX];
-#pragma unroll
-            for (int j = 0; j < LX; ++j) {
-                float acc = 0.f;
-#pragma unroll
-                for (int k = 0; k < W; ++k) acc = fmaf(gw.w[k], v[OFF + j + k], acc);
-                o[j] = acc;
-            }
-            float4* xp = reinterpret_cast<float4*>(X + (cc * PY + r) * XP + g * LX);
-#pragma unroll
-            for (int q4 = 0; q4 < LX / 4; ++q4) xp[q4] = make_float4(o[4 * q4], o[4 * q4 + 1], o[4 * q4 + 2], o[4 * q4 + 3]);
         }
         __syncthreads();
         px0 = x0; py0 = y0; pz = z; have_prev = true;
