@@ -24,9 +24,6 @@ static int pick_chunk(int n, int min_chunk, long long ctas_per_chunk, long long 
     return chunk;
 }
 
-#ifndef DISC_FG_TYBIG
-#define DISC_FG_TYBIG 32
-#endif
 template <int K, int FORCE, int TY>
 static void launch_fg_t4(const DevInfo& di, const float* m, const float* s, const float* rin, float* rout, int nx, int ny,
                          int nz, float eps_den, const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
@@ -53,7 +50,7 @@ static void launch_fg(const DevInfo& di, const float* m, const float* s, const f
         if (tiles32 < (long long)FgT4Cfg<K, 32>::OCC * n_sm)
             launch_fg_t4<K, FORCE, 8>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
         else
-            launch_fg_t4<K, FORCE, DISC_FG_TYBIG>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
+            launch_fg_t4<K, FORCE, 32>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
         return;
     }
     const int txb = nx > 64 ? 128 : (nx > 32 ? 64 : 32);

@@ -68,8 +68,11 @@ def test_warp(disc, oracle_mod, shape):
 
 # ------------------------------------------------------------------ moments
 @pytest.mark.parametrize("R", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10])
+# Which kernel a case reaches (csrc/moments_tu.cu): nx % 4 != 0 -> the plain-load kernels; nx % 4 == 0 and at most two
+# waves of 32x8x4 blocks (the first four such shapes, R <= 6) -> the block kernel of the coarse levels; nx % 4 == 0
+# and either R >= 7 or more blocks than that (the last shape) -> the marching TMA + tensor-memory kernel.
 @pytest.mark.parametrize("shape", [(7, 6, 5), (20, 45, 70), (37, 18, 33), (20, 45, 72), (37, 18, 36), (3, 5, 8),
-                                   (26, 50, 100)])
+                                   (26, 50, 100), (40, 100, 132)])
 def test_box_moments(disc, oracle_mod, shape, R):
     vol, _ = rand_pair(shape, 20 + R)
     ctx = make_ctx(disc, shape, R=R)
@@ -95,7 +98,8 @@ def test_box_moments_constant_volume_has_zero_variance(disc):
 
 # ------------------------------------------------------------------ correction
 @pytest.mark.parametrize("R", [0, 1, 3, 5, 7, 10])
-@pytest.mark.parametrize("shape", [(7, 6, 5), (20, 45, 70), (37, 18, 33), (20, 45, 72), (37, 18, 36), (26, 50, 100)])
+@pytest.mark.parametrize("shape", [(7, 6, 5), (20, 45, 70), (37, 18, 33), (20, 45, 72), (37, 18, 36), (26, 50, 100),
+                                   (40, 100, 132)])
 def test_correct_intensity(disc, oracle_mod, shape, R):
     m, s = rand_pair(shape, 30 + R)
     ctx = make_ctx(disc, shape, R=R)
