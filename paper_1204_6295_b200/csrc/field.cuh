@@ -83,7 +83,7 @@ __device__ __forceinline__ void force_increment(const float* __restrict__ m, con
 
 // NEXT-3, the paper's "comparison kernel": sum_x |dr(x)| and sum_x |r(x)| (Euclidean norm per
 // voxel, reading A16) of iteration `iter`, per-thread fp32 norms accumulated in fp64.  Every block writes its two
-// partial sums to its own slot; the last block to finish adds them IN BLOCK ORDER (so l, and with it the iteration the
+// partial sums to its own slot; the last block to finish adds them in a fixed association (so l, and with it the iteration the
 // level stops at, is the same from run to run), forms l = sum|dr| / sum|r| (+inf while the field is zero), files it in
 // the 16-slot history and, from iteration 10 on, sets stop_iter = iter when l(iter-10) - l(iter) <= stop_eps.  Kernels
 // of later iterations then fall through.
@@ -120,15 +120,30 @@ k_force_norms(const float* __restrict__ m, const float* __restrict__ s, const fl
         last = atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1;
     }
     __syncthreads();
-    if (last && threadIdx.x == 0) {
+    if (last) {
+        // the last block adds the partials in a FIXED association (thread i takes blocks i, i + 256, ... in rising order,
+        // then a fixed tree over the 256 threads), so l -- and the iteration a level stops at -- is the same from run
+        // to run, without one thread walking up to 2048 partials through L2 one after the other
         __threadfence();
         double sdr = 0.0, sr = 0.0;
-        for (unsigned k = 0; k < gridDim.x; ++k) { sdr += ctl->partial[2 * k]; sr += ctl->partial[2 * k + 1]; }
-        const double l = sr > 0.0 ? sdr / sr : (double)INFINITY;
-        ctl->hist[iter & 15] = l;
-        if (iter >= 10 && ctl->hist[(iter - 10) & 15] - l <= (double)stop_eps) ctl->stop_iter = iter;
-        ctl->ticket = 0u;
-        __threadfence();
+        for (unsigned k = threadIdx.x; k < gridDim.x; k += blockDim.x) { sdr += ctl->partial[2 * k]; sr += ctl->partial[2 * k + 1]; }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            sdr += __shfl_xor_sync(0xffffffffu, sdr, o);
+            sr += __shfl_xor_sync(0xffffffffu, sr, o);
+        }
+        __syncthreads();                      // sh[] of the first reduction has been read by thread 0
+        if (lane == 0) { sh[0][warp] = sdr; sh[1][warp] = sr; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            sdr = 0.0; sr = 0.0;
+            for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { sdr += sh[0][w]; sr += sh[1][w]; }
+            const double l = sr > 0.0 ? sdr / sr : (double)INFINITY;
+            ctl->hist[iter & 15] = l;
+            if (iter >= 10 && ctl->hist[(iter - 10) & 15] - l <= (double)stop_eps) ctl->stop_iter = iter;
+            ctl->ticket = 0u;
+            __threadfence();
+        }
     }
 }
 
