@@ -156,7 +156,7 @@ class Ctx:
 
     def __del__(self):
         h, self.handle = getattr(self, "handle", None), None
-        if h:
+        if h and _lib is not None:     # at interpreter shutdown the module globals may already be gone
             _lib.disc_destroy(h)
 
 

@@ -85,6 +85,25 @@ def test_box_moments(disc, oracle_mod, shape, R):
     assert var.min().item() >= 0.0
 
 
+# the block kernel of the coarse levels (csrc/moments_blk.cuh): blocks of 32 x 8 x 4 outputs (32 x 8 x 2 at R = 6) with
+# ragged edges in every axis, volumes thinner than one block or than the patch, a single row, and all three modes
+@pytest.mark.parametrize("R", [0, 1, 5, 6])
+@pytest.mark.parametrize("shape", [(1, 1, 4), (2, 9, 12), (5, 8, 64), (9, 13, 36), (6, 3, 40)])
+def test_block_kernel_edge_shapes(disc, oracle_mod, shape, R):
+    vol, other = rand_pair(shape, 70 + R)
+    ctx = make_ctx(disc, shape, R=R)
+    mean = torch.empty(shape, device="cuda"); var = torch.empty(shape, device="cuda"); out = torch.empty(shape, device="cuda")
+    disc.disc_box_moments(ctx, 0, dev(vol), mean, var)
+    rm, rv = oracle_mod.box_moments(vol, R)
+    rngv = max(float(vol.max() - vol.min()), 1.0)
+    assert np.abs(mean.cpu().numpy() - rm).max() <= 1e-4 * rngv
+    assert np.abs(np.sqrt(var.cpu().numpy().astype(np.float64)) - np.sqrt(rv)).max() <= 1e-4 * rngv
+    disc.disc_correct_intensity(ctx, 0, dev(other), dev(vol), out)          # z-score of `other`, then the correction
+    ref = oracle_mod.correct(other, vol, R)
+    tol = 1e-4 * max(float(max(vol.max(), other.max()) - min(vol.min(), other.min())), 1.0)
+    assert np.abs(out.cpu().numpy() - ref).max() <= tol
+
+
 def test_box_moments_constant_volume_has_zero_variance(disc):
     """the H1 hazard: E(x^2) - mu^2 must not leak rounding into var (fp32 sums give ~9 HU^2 here)"""
     shape = (24, 40, 72)
