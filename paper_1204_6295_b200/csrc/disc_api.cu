@@ -160,6 +160,11 @@ disc_status launch_downsample(disc_ctx* c, const Level& fine, const float* in, f
 disc_status launch_upsample(disc_ctx* c, const Level& coarse, const float* in, float* out, cudaStream_t st) {
     const int* f = c->fac;
     const int nx = f[0] * coarse.nx, ny = f[1] * coarse.ny, nz = f[2] * coarse.nz;
+    if (f[0] == 2 && f[1] == 2 && f[2] == 2 && (reinterpret_cast<uintptr_t>(out) & 7u) == 0) {   // 8-byte stores of x pairs
+        dim3 grid2((coarse.nx + 127) / 128, coarse.ny, 3 * coarse.nz);
+        k_upsample_field_222<<<grid2, 128, 0, st>>>(in, out, coarse.nx, coarse.ny, coarse.nz);
+        return check_launch(c, "k_upsample_field_222");
+    }
     dim3 grid((nx + 127) / 128, ny, 3 * nz);
     k_upsample_field<<<grid, 128, 0, st>>>(in, out, coarse.nx, coarse.ny, coarse.nz, f[0], f[1], f[2]);
     return check_launch(c, "k_upsample_field");
