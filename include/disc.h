@@ -116,9 +116,9 @@ disc_status disc_set_force(disc_ctx* ctx, int mode);
  * l = +inf while the field is zero).  The first iteration k >= 10 with  l(k-10) - l(k) <= eps  is completed and is the
  * level's last; `iters` of disc_create stays the per-level maximum.  (The text's condition is followed; Alg. A1's
  * `while` prints it inverted.)  The paper's value is eps = 1e-4.
- * The test runs on the device: one extra launch per iteration (the paper's "comparison kernel", reading m, s', r once
- * more: +20 B/voxel) whose last block sets a flag; the kernels of the remaining iterations are still enqueued but
- * return at once, so there is no host synchronisation.  Host-side state only, no launch. */
+ * The test runs on the device (the paper's "comparison kernel"): the force kernel of the iteration adds the two sums up
+ * while it evaluates the force, and its last block sets a flag; the kernels of the remaining iterations are still
+ * enqueued but return at once, so there is no host synchronisation.  Host-side state only, no launch. */
 disc_status disc_set_stop(disc_ctx* ctx, float eps);
 
 /*

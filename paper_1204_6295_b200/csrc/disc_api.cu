@@ -125,9 +125,9 @@ disc_status launch_moments(disc_ctx* c, const Level& L, const float* vol, const 
 
 // force: 0 = plain smoothing, otherwise the context's force mode
 disc_status launch_force_gxy(disc_ctx* c, bool force, const Level& L, const float* m, const float* s, const float* rin,
-                             float* rout, IterCtl ctl, cudaStream_t st) {
+                             float* rout, IterCtl ctl, cudaStream_t st, StopReq stop = StopReq{nullptr, 0, 0.f}) {
     const int FORCE = force ? c->force_mode : 0;
-    if (!launch_force_gxy_any(c->di, c->K, FORCE, m, s, rin, rout, L.nx, L.ny, L.nz, DISC_EPS_DEN, c->taps, ctl, st))
+    if (!launch_force_gxy_any(c->di, c->K, FORCE, m, s, rin, rout, L.nx, L.ny, L.nz, DISC_EPS_DEN, c->taps, ctl, stop, st))
         return fail(c, DISC_ERR_UNSUPPORTED, "Gaussian radius %d unsupported", c->K);
     return check_launch(c, "k_force_gxy");
 }
@@ -269,12 +269,10 @@ disc_status iterate_level(disc_ctx* c, Level& L, const float* ct, const float* c
             rc = launch_moments<kModeCorrect>(c, L, L.m, L.zhat, L.sp, nullptr, ctl, st);     // A1 steps 1,3
             if (rc == DISC_OK && slot >= 0) rc = correct_ab(c, L, cbct, L.m, nullptr, false, slot, ctl, st);   // Fig. 9 only
         }
-        if (rc == DISC_OK && stop) {                                                           // PAPER.md:167, l^(k)
-            launch_force_norms(c->force_mode, L.m, L.sp, disp, L.nx, L.ny, L.nz, DISC_EPS_DEN, c->d_stop, k, c->stop_eps,
-                               c->di.n_sm, st);
-            rc = check_launch(c, "k_force_norms");
-        }
-        if (rc == DISC_OK) rc = launch_force_gxy(c, true, L, L.m, L.sp, disp, L.scratch, ctl, st);  // A1 steps 4,5,6(x,y)
+        // A1 steps 4,5,6(x,y); with the criterion on, the same kernel adds up sum|dr|, sum|r| of the iteration and its
+        // last block takes the decision (l^(k)): kernels of later iterations fall through
+        const StopReq sreq = stop ? StopReq{c->d_stop, k, c->stop_eps} : StopReq{nullptr, 0, 0.f};
+        if (rc == DISC_OK) rc = launch_force_gxy(c, true, L, L.m, L.sp, disp, L.scratch, ctl, st, sreq);
         if (rc == DISC_OK) {
             if (k + 1 < n_iters || final_warp)
                 rc = launch_gz_warp<true>(c, L, L.scratch, disp, ct, L.m, ctl, st);            // A1 step 6(z) + next I_m^(k)

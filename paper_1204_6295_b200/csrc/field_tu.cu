@@ -24,23 +24,33 @@ static int pick_chunk(int n, int min_chunk, long long ctas_per_chunk, long long 
     return chunk;
 }
 
-template <int K, int FORCE, int TY>
-static void launch_fg_t4(const DevInfo& di, const float* m, const float* s, const float* rin, float* rout, int nx, int ny,
-                         int nz, float eps_den, const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
+template <int K, int FORCE, int TY, bool STOP>
+static void launch_fg_t4s(const DevInfo& di, const float* m, const float* s, const float* rin, float* rout, int nx, int ny,
+                          int nz, float eps_den, const GaussTaps& taps, IterCtl ctl, StopReq stop, cudaStream_t st) {
     using C = FgT4Cfg<K, TY>;
     static bool configured[kMaxDevices] = {};  // the opt-in is per device (idempotent, so a race is harmless)
     if (!configured[di.dev]) {
-        cudaFuncSetAttribute(k_force_gxy_t4<K, FORCE, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
+        cudaFuncSetAttribute(k_force_gxy_t4<K, FORCE, TY, STOP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
         configured[di.dev] = true;
     }
     const long long n_tiles = (long long)((nx + C::TX - 1) / C::TX) * ((ny + C::TY - 1) / C::TY) * nz;
     const int grid = (int)(n_tiles < (long long)C::OCC * di.n_sm ? n_tiles : (long long)C::OCC * di.n_sm);   // persistent: OCC CTAs per SM
-    k_force_gxy_t4<K, FORCE, TY><<<grid, C::NT, C::smem_bytes, st>>>(m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl);
+    k_force_gxy_t4<K, FORCE, TY, STOP><<<grid, C::NT, C::smem_bytes, st>>>(m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, stop.ctl,
+                                                                         stop.iter, stop.eps);
+}
+
+template <int K, int FORCE, int TY>
+static void launch_fg_t4(const DevInfo& di, const float* m, const float* s, const float* rin, float* rout, int nx, int ny,
+                         int nz, float eps_den, const GaussTaps& taps, IterCtl ctl, StopReq stop, cudaStream_t st) {
+    if constexpr (FORCE != 0) {
+        if (stop.ctl) { launch_fg_t4s<K, FORCE, TY, true>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, stop, st); return; }
+    }
+    launch_fg_t4s<K, FORCE, TY, false>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, stop, st);
 }
 
 template <int K, int FORCE>
 static void launch_fg(const DevInfo& di, const float* m, const float* s, const float* rin, float* rout, int nx, int ny,
-                      int nz, float eps_den, const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
+                      int nz, float eps_den, const GaussTaps& taps, IterCtl ctl, StopReq stop, cudaStream_t st) {
     const bool vec_ok = nx % 4 == 0 && aligned16(rin) && aligned16(rout) && (!FORCE || (aligned16(m) && aligned16(s))) &&
                         3ull * nx * ny * nz < 0xffffffffull;   // the tile kernel indexes voxels with 32 bits
     const int n_sm = di.n_sm;
@@ -48,11 +58,14 @@ static void launch_fg(const DevInfo& di, const float* m, const float* s, const f
         // 64 x 32 tiles; 64 x 8 where those would leave CTA slots of the device empty (small levels)
         const long long tiles32 = (long long)((nx + 63) / 64) * ((ny + 31) / 32) * nz;
         if (tiles32 < (long long)FgT4Cfg<K, 32>::OCC * n_sm)
-            launch_fg_t4<K, FORCE, 8>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
+            launch_fg_t4<K, FORCE, 8>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, stop, st);
         else
-            launch_fg_t4<K, FORCE, 32>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
+            launch_fg_t4<K, FORCE, 32>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, stop, st);
         return;
     }
+    // plain-load fallback: the criterion's sums come from their own pass over m, s', r
+    if (FORCE != 0 && stop.ctl)
+        launch_force_norms(FORCE, m, s, rin, nx, ny, nz, eps_den, stop.ctl, stop.iter, stop.eps, n_sm, st);
     const int txb = nx > 64 ? 128 : (nx > 32 ? 64 : 32);
     const int xt = (nx + txb - 1) / txb;
     const int yseg = pick_chunk(ny, 8 * K > 32 ? 8 * K : 32, (long long)xt * nz, 4LL * n_sm);
@@ -104,11 +117,11 @@ static void launch_gz(const DevInfo& di, const float* rin, float* rout, const fl
 // one Gaussian radius: launches if K lies in this unit's range (the discarded branch is never instantiated)
 template <int K>
 static bool case_fg(const DevInfo& di, int force, const float* m, const float* s, const float* rin, float* rout, int nx,
-                    int ny, int nz, float eps_den, const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
+                    int ny, int nz, float eps_den, const GaussTaps& taps, IterCtl ctl, StopReq stop, cudaStream_t st) {
     if constexpr (K >= DISC_K_LO && K <= DISC_K_HI) {
-        if (force == kForceDouble) launch_fg<K, kForceDouble>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
-        else if (force == kForceSingle) launch_fg<K, kForceSingle>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
-        else launch_fg<K, kForceNone>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
+        if (force == kForceDouble) launch_fg<K, kForceDouble>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, stop, st);
+        else if (force == kForceSingle) launch_fg<K, kForceSingle>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, stop, st);
+        else launch_fg<K, kForceNone>(di, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, stop, st);
         return true;
     } else {
         return false;
@@ -131,10 +144,10 @@ static bool case_gz(const DevInfo& di, bool warp, const float* rin, float* rout,
 
 bool DISC_CAT(launch_force_gxy_tu, DISC_TU)(const DevInfo& di, int K, int force, const float* m, const float* s,
                                             const float* rin, float* rout, int nx, int ny, int nz, float eps_den,
-                                            const GaussTaps& taps, IterCtl ctl, cudaStream_t st) {
+                                            const GaussTaps& taps, IterCtl ctl, StopReq stop, cudaStream_t st) {
     switch (K) {
 #define DISC_CASE(k) \
-    case k: return case_fg<k>(di, force, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
+    case k: return case_fg<k>(di, force, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, stop, st);
         DISC_FOR_K(DISC_CASE)
 #undef DISC_CASE
     }
@@ -198,11 +211,11 @@ bool launch_moments_any(const DevInfo& di, int rxy, int rz, int mode, const floa
 
 bool launch_force_gxy_any(const DevInfo& di, int K, int force, const float* m, const float* s, const float* rin,
                           float* rout, int nx, int ny, int nz, float eps_den, const GaussTaps& taps, IterCtl ctl,
-                          cudaStream_t st) {
-    return launch_force_gxy_tu0(di, K, force, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st) ||
-           launch_force_gxy_tu1(di, K, force, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st) ||
-           launch_force_gxy_tu2(di, K, force, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st) ||
-           launch_force_gxy_tu3(di, K, force, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, st);
+                          StopReq stop, cudaStream_t st) {
+    return launch_force_gxy_tu0(di, K, force, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, stop, st) ||
+           launch_force_gxy_tu1(di, K, force, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, stop, st) ||
+           launch_force_gxy_tu2(di, K, force, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, stop, st) ||
+           launch_force_gxy_tu3(di, K, force, m, s, rin, rout, nx, ny, nz, eps_den, taps, ctl, stop, st);
 }
 
 bool launch_gz_warp_any(const DevInfo& di, int K, bool warp, const float* rin, float* rout, const float* moving,

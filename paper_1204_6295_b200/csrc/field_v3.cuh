@@ -349,7 +349,10 @@ struct FgGroup {
     // Two points at a time (x-adjacent halves of the 16-byte loads) with packed fp32x2 arithmetic: the same operations
     // in the same order as the scalar form, so every half rounds identically; only the x differences, whose operands
     // straddle the halves, and the two reciprocals are scalar.
-    __device__ __forceinline__ void finish(float eps_den) {
+    // NORMS (stopping criterion; reading A16): also the sums over the four points of |dr| (the increment
+    // about to be added, Euclidean norm) and |r| (the field before the update), as k_force_norms forms them.
+    template <bool NORMS>
+    __device__ __forceinline__ void finish(float eps_den, float& sum_dr, float& sum_r) {
         if (FORCE) {
             const float2 eps4 = make_float2(4.f * eps_den, 4.f * eps_den);
             const float2 scp[2] = {make_float2(sc.x, sc.y), make_float2(sc.z, sc.w)};
@@ -370,6 +373,12 @@ struct FgGroup {
                 const float2 tt = ffma2(t, t, eps4);
                 const float2 den = ffma2(Dx, Dx, ffma2(Dy, Dy, ffma2(Dz, Dz, tt)));
                 const float2 q = fmul2(t, make_float2(rcp_approx(den.x), rcp_approx(den.y)));
+                float2 ax, ay, az;      // the increment itself, for its norm
+                if (NORMS) {
+                    const float2 r2 = ffma2(up[0][h], up[0][h], ffma2(up[1][h], up[1][h], fmul2(up[2][h], up[2][h])));
+                    sum_r += sqrt_approx(r2.x) + sqrt_approx(r2.y);
+                    ax = fmul2(q, Dx); ay = fmul2(q, Dy); az = fmul2(q, Dz);
+                }
                 up[0][h] = ffma2(q, Dx, up[0][h]);
                 up[1][h] = ffma2(q, Dy, up[1][h]);
                 up[2][h] = ffma2(q, Dz, up[2][h]);
@@ -381,9 +390,14 @@ struct FgGroup {
                                              : fsub2(make_float2(mzp.z, mzp.w), make_float2(mzm.z, mzm.w));
                     const float2 dh = ffma2(Hx, Hx, ffma2(Hy, Hy, ffma2(Hz, Hz, tt)));
                     const float2 p = fmul2(t, make_float2(rcp_approx(dh.x), rcp_approx(dh.y)));
+                    if (NORMS) { ax = ffma2(p, Hx, ax); ay = ffma2(p, Hy, ay); az = ffma2(p, Hz, az); }
                     up[0][h] = ffma2(p, Hx, up[0][h]);
                     up[1][h] = ffma2(p, Hy, up[1][h]);
                     up[2][h] = ffma2(p, Hz, up[2][h]);
+                }
+                if (NORMS) {
+                    const float2 n2 = ffma2(ax, ax, ffma2(ay, ay, fmul2(az, az)));
+                    sum_dr += sqrt_approx(n2.x) + sqrt_approx(n2.y);
                 }
             }
 #pragma unroll
@@ -398,11 +412,17 @@ struct FgGroup {
 // running at the same time work on neighbouring tiles and share their halos in L2).  Phase 3 of tile t-1 and
 // phase 1 of tile t share one barrier interval -- the y pass (pure FMA work out of shared memory) runs on some
 // warps while others wait for phase 1's global loads.
-template <int K, int FORCE, int TY_>
+// STOP (the paper's "comparison kernel"): phase 1 also adds up sum|dr| and sum|r| over
+// the voxels of the tile proper (every voxel belongs to exactly one tile), per thread in fp64; every CTA leaves its two
+// partial sums in its own slot and the last CTA to finish adds them in a fixed association, forms l = sum|dr| / sum|r|,
+// files it and sets stop_iter when l(iter-10) - l(iter) <= stop_eps -- no second pass over m, s', r.
+template <int K, int FORCE, int TY_, bool STOP>
 __global__ void __launch_bounds__(FgT4Cfg<K, TY_>::NT, FgT4Cfg<K, TY_>::OCC)
 k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const float* __restrict__ rin,
-               float* __restrict__ rout, int nx, int ny, int nz, float eps_den, GaussTaps gw, IterCtl ctl) {
+               float* __restrict__ rout, int nx, int ny, int nz, float eps_den, GaussTaps gw, IterCtl ctl,
+               StopCtl* sctl, int stop_iter_k, float stop_eps) {
     if (iter_skipped(ctl)) return;
+    double acc_dr = 0.0, acc_r = 0.0;
     using C = FgT4Cfg<K, TY_>;
     constexpr int W = C::W, TX = C::TX, TY = C::TY, NT = C::NT, LX = C::LX, LY = C::LY, NG = C::NG, NRP = C::NRP;
     constexpr int UPP = C::UPP, XP = C::XP, XPP = C::XPP, KA = C::KA, NV = C::NV;
@@ -459,8 +479,18 @@ k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const f
                             G1.mym = adj ? G0.mm : mym0;
                         }
                     }
-                    G0.finish(eps_den);
-                    G1.finish(eps_den);
+                    float ndr0 = 0.f, nr0 = 0.f, ndr1 = 0.f, nr1 = 0.f;
+                    G0.template finish<STOP>(eps_den, ndr0, nr0);
+                    G1.template finish<STOP>(eps_den, ndr1, nr1);
+                    if (STOP) {
+                        // a group is wholly inside or wholly outside the tile proper and the volume (x0, KA, nx are multiples of 4)
+                        const bool in_x = gx >= x0 && gx < x0 + TX && gx < nx;
+                        const int rr = 2 * rp - K;
+                        const bool in0 = in_x && rr >= 0 && rr < TY && y0 + rr < ny;
+                        const bool in1 = in_x && rr + 1 >= 0 && rr + 1 < TY && y0 + rr + 1 < ny;
+                        acc_dr += (double)((in0 ? ndr0 : 0.f) + (in1 ? ndr1 : 0.f));
+                        acc_r += (double)((in0 ? nr0 : 0.f) + (in1 ? nr1 : 0.f));
+                    }
                     // a group wholly outside the volume is the replicate border: the edge group's outermost value
                     if (gx < 0 || gx >= nx) {   // only in the tiles at the volume's x border
 #pragma unroll
@@ -554,6 +584,48 @@ k_force_gxy_t4(const float* __restrict__ m, const float* __restrict__ s, const f
         }
         __syncthreads();
         px0 = x0; py0 = y0; pz = z; have_prev = true;
+    }
+    if (STOP) {
+        const int lane = tid & 31, warp = tid >> 5;
+        __shared__ double sh[2][NT / 32];
+        __shared__ bool last;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            acc_dr += __shfl_xor_sync(0xffffffffu, acc_dr, o);
+            acc_r += __shfl_xor_sync(0xffffffffu, acc_r, o);
+        }
+        if (lane == 0) { sh[0][warp] = acc_dr; sh[1][warp] = acc_r; }
+        __syncthreads();
+        if (tid == 0) {
+            double ta = 0.0, tb = 0.0;
+            for (int w = 0; w < NT / 32; ++w) { ta += sh[0][w]; tb += sh[1][w]; }
+            sctl->partial[2 * blockIdx.x] = ta; sctl->partial[2 * blockIdx.x + 1] = tb;
+            __threadfence();
+            last = atomicAdd(&sctl->ticket, 1u) == gridDim.x - 1;
+        }
+        __syncthreads();
+        if (last) {   // fixed association: thread i takes CTAs i, i + NT, ... in rising order, then a fixed tree
+            __threadfence();
+            double sdr = 0.0, sr = 0.0;
+            for (unsigned k = tid; k < gridDim.x; k += NT) { sdr += sctl->partial[2 * k]; sr += sctl->partial[2 * k + 1]; }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                sdr += __shfl_xor_sync(0xffffffffu, sdr, o);
+                sr += __shfl_xor_sync(0xffffffffu, sr, o);
+            }
+            __syncthreads();
+            if (lane == 0) { sh[0][warp] = sdr; sh[1][warp] = sr; }
+            __syncthreads();
+            if (tid == 0) {
+                sdr = 0.0; sr = 0.0;
+                for (int w = 0; w < NT / 32; ++w) { sdr += sh[0][w]; sr += sh[1][w]; }
+                const double l = sr > 0.0 ? sdr / sr : (double)INFINITY;
+                sctl->hist[stop_iter_k & 15] = l;
+                if (stop_iter_k >= 10 && sctl->hist[(stop_iter_k - 10) & 15] - l <= (double)stop_eps) sctl->stop_iter = stop_iter_k;
+                sctl->ticket = 0u;
+                __threadfence();
+            }
+        }
     }
 }
 

@@ -24,6 +24,15 @@ enum MomentsMode {
     kModeCorrect = 2   // out0 = sigma_m * aux + mu_m  (aux = CBCT z-score)          (per-iteration correction)
 };
 
+// The stopping criterion's request to the force kernel of iteration `iter` (ctl == nullptr: criterion off): the fused
+// tile kernel adds sum|dr|, sum|r| up itself (block partials, last block decides); the plain-load fallback launches
+// k_force_norms first.
+struct StopReq {
+    StopCtl* ctl;
+    int iter;
+    float eps;
+};
+
 // sum|dr|, sum|r| of the iteration -> l^(k), criterion check in the last block (field.cuh k_force_norms)
 void launch_force_norms(int force, const float* m, const float* s, const float* r, int nx, int ny, int nz, float eps_den,
                         StopCtl* ctl, int iter, float stop_eps, int n_sm, cudaStream_t st);
@@ -37,7 +46,7 @@ bool launch_moments_any(const DevInfo& di, int rxy, int rz, int mode, const floa
 // force = 0 none (plain smoothing), 1 Thirion / passive, 2 double (ForceMode in field.cuh)
 bool launch_force_gxy_any(const DevInfo& di, int K, int force, const float* m, const float* s, const float* rin,
                           float* rout, int nx, int ny, int nz, float eps_den, const GaussTaps& taps, IterCtl ctl,
-                          cudaStream_t st);
+                          StopReq stop, cudaStream_t st);
 bool launch_gz_warp_any(const DevInfo& di, int K, bool warp, const float* rin, float* rout, const float* moving,
                         float* mout, int nx, int ny, int nz, const GaussTaps& taps, IterCtl ctl, cudaStream_t st);
 void launch_force_update(int force, const float* m, const float* s, float* r, int nx, int ny, int nz, float eps_den,
@@ -51,7 +60,7 @@ void launch_warp_kernel(const float* moving, const float* r, float* out, int nx,
                               cudaStream_t st);                                                                          \
     bool launch_force_gxy_tu##n(const DevInfo& di, int K, int force, const float* m, const float* s, const float* rin,  \
                                 float* rout, int nx, int ny, int nz, float eps_den, const GaussTaps& taps, IterCtl ctl, \
-                                cudaStream_t st);                                                                        \
+                                StopReq stop, cudaStream_t st);                                                                        \
     bool launch_gz_warp_tu##n(const DevInfo& di, int K, bool warp, const float* rin, float* rout, const float* moving,  \
                               float* mout, int nx, int ny, int nz, const GaussTaps& taps, IterCtl ctl, cudaStream_t st);
 DISC_DECL_TU(0) DISC_DECL_TU(1) DISC_DECL_TU(2) DISC_DECL_TU(3)

@@ -120,12 +120,6 @@ __device__ __forceinline__ float rsqrt_nr(float v) {
     return y * fmaf(-0.5f * v * y, y, 1.5f);
 }
 
-__device__ __forceinline__ float sqrt_approx(float v) {
-    float y;
-    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(v));
-    return y;
-}
-
 template <int R, int TY, int MODE>
 __global__ void __launch_bounds__(MomV3Cfg<R, TY>::NT, 1)
 k_moments_v3(const __grid_constant__ CUtensorMap tmap, const float* __restrict__ pv, float* __restrict__ out0,
