@@ -127,6 +127,8 @@ def test_register_double_force(disc, oracle_mod, dims, R, sigma, levels, iters):
     ((64, 64, 32), 3, 1.5, 1, 50, 4e-2, False),      # config 1's schedule with the criterion on (trips at k = 32)
     ((48, 40, 24), 2, 2.0, 2, 30, 5e-3, True),
     ((40, 36, 20), 2, 1.5, 2, 14, 1e-4, False),      # the paper's eps: nothing trips, all iterations run
+    ((44, 40, 24), 2, 1.5, 2, 30, 3e-3, False),      # nx = 22 at the coarse level: the plain-load force kernel, whose
+                                                     # sums come from the separate k_force_norms launch
 ])
 def test_register_stopping_criterion(disc, oracle_mod, dims, R, sigma, levels, iters, eps, double_force):
     """NEXT-3: the device-side criterion stops each level where the oracle's does.  The decision
