@@ -244,3 +244,31 @@ def test_argument_errors(disc):
     with pytest.raises(disc.DiscError):
         disc.disc_upsample_field(ctx, 0, torch.zeros(3 * 512, device="cuda"), torch.zeros(3 * 4096, device="cuda"))
     assert "level" in disc.disc_last_error(ctx)
+
+
+# ------------------------------------------------------------------ run-to-run reproducibility
+@pytest.mark.parametrize("shape,R,sigma", [((32, 64, 64), 5, 2.0), ((26, 50, 100), 3, 1.5), ((9, 13, 36), 6, 1.0),
+                                           ((40, 100, 132), 2, 2.5)])
+def test_kernels_are_bit_reproducible(disc, shape, R, sigma):
+    """Every kernel is a deterministic function of its inputs, so repeated launches must agree bit for bit.  A buffer
+    released to its producer while loads from it are still in flight (the race the moments kernel once had, DESIGN.md
+    section 8) or a shared-memory hazard between the phases of the tile kernels shows up here as a differing output."""
+    rng = np.random.default_rng(5)
+    nz, ny, nx = shape
+    a, b = rand_pair(shape, 90)
+    r0 = rng.uniform(-2, 2, size=(3,) + shape).astype(np.float32)
+    ctx = make_ctx(disc, shape, R=R, sigma=sigma)
+    da, db = dev(a), dev(b)
+    ref = {}
+    for it in range(60):
+        out = torch.empty(shape, device="cuda"); disc.disc_correct_intensity(ctx, 0, db, da, out)
+        mean = torch.empty(shape, device="cuda"); var = torch.empty(shape, device="cuda")
+        disc.disc_box_moments(ctx, 0, da, mean, var)
+        r = dev(r0)
+        disc.disc_demons_step(ctx, 0, da, db, r)
+        for k, v in (("corrected", out), ("mean", mean), ("var", var), ("step", r)):
+            if it == 0:
+                ref[k] = v.clone()
+            else:
+                assert torch.equal(ref[k], v), (k, it)
+    disc.disc_destroy(ctx)
