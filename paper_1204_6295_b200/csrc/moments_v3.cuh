@@ -146,8 +146,19 @@ k_moments_v3(const __grid_constant__ CUtensorMap tmap, const float* __restrict__
     const int T = zlast - zfirst + 1;
     const uint32_t tmem_cols = pow2_tmem_cols((uint32_t)(C::GROUPS * C::RING_WORDS * wz));
 
-    if (tid == 0) {
+    // The producer thread sets up its own barriers and has the first NSTG slices on their way before the CTA-wide
+    // sync: the first load's latency (tensor-map fetch + DRAM) then overlaps the tensor-memory allocation, the zeroing
+    // of the ring and the fp64 divisions of the set-up instead of following them.
+    const int n_first = min(NSTG, T);
+    if (tid == NYZ + 32 * NXW) {
         for (int i = 0; i < NSTG; ++i) { mbar_init(&raw_full[i], 1); mbar_init(&raw_empty[i], PY); }
+        mbar_fence_init();
+        for (int t = 0; t < n_first; ++t) {
+            mbar_expect_tx(&raw_full[t], (uint32_t)C::raw_bytes);
+            tma_load_3d(raw + t * RAWS, &tmap, x0 - C::RA, y0 - R, zfirst + t, &raw_full[t]);
+        }
+    }
+    if (tid == 0) {
         for (int i = 0; i < NXS; ++i) { mbar_init(&xs_full[i], PY); mbar_init(&xs_empty[i], NYZ); }
         mbar_fence_init();
     }
@@ -346,9 +357,9 @@ k_moments_v3(const __grid_constant__ CUtensorMap tmap, const float* __restrict__
         }
     } else if (tid == NYZ + 32 * NXW) {
         // ------------------------------------------------------------------ producer
-        for (int t = 0; t < T; ++t) {
+        for (int t = n_first; t < T; ++t) {
             const int st = t % NSTG;
-            if (t >= NSTG) mbar_wait(&raw_empty[st], ((t / NSTG) - 1) & 1);
+            mbar_wait(&raw_empty[st], ((t / NSTG) - 1) & 1);
             mbar_expect_tx(&raw_full[st], (uint32_t)C::raw_bytes);
             tma_load_3d(raw + st * RAWS, &tmap, x0 - C::RA, y0 - R, zfirst + t, &raw_full[st]);
         }
