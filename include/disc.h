@@ -90,8 +90,8 @@ disc_status disc_create_ex(disc_ctx** out, const int dims[3], const float spacin
 /* Synchronises the device, frees the context and its scratch.  NULL is allowed. */
 void disc_destroy(disc_ctx* ctx);
 
-/* Message of the last error of this context (or of the last failed disc_create when ctx == NULL).
- * The string is owned by the library and valid until the next call on the same context. */
+/* Message of the last error of this context (ctx == NULL: of the calling thread's last failed disc_create or
+ * disc_smooth_field_noalloc).  The string is owned by the library and valid until the next call on the same context. */
 const char* disc_last_error(const disc_ctx* ctx);
 
 /* Number of CUDA kernels this context has launched so far (bench.py's gpu_launches). */
@@ -233,6 +233,41 @@ disc_status disc_downsample(disc_ctx* ctx, int level_from, const float* vol, flo
 /* Up-sampling of a field from level_from to level_from-1: trilinear at i/2 - 1/4 (clamped) with the value doubled
  * along every axis the pyramid halves (reading A9).  disp [3*N_level_from], out [3*N_level_from-1]. */
 disc_status disc_upsample_field(disc_ctx* ctx, int level_from, const float* disp, float* out, void* stream);
+
+/* ---- an entry point for callers that are not allowed to allocate device memory ---- */
+
+/*
+ * disc_smooth_field_noalloc -- step (d), disp_inout <- G_sigma * disp_inout (readings A3, A10), computed by
+ * the same two kernels as disc_smooth_field and bit-identical to it, but WITHOUT a context and without any allocation.
+ *
+ * Who needs it.  Every other compute call needs a disc_ctx, and disc_create obtains the scratch of all kernels with
+ * cudaMalloc.  Some hosts of this library cannot do that: an application that carves the GPU's memory up itself at
+ * start-up and forbids library-side cudaMalloc, or a latency-bound treatment-room loop (re-regularising a field between
+ * two beam deliveries) in which cudaMalloc / cudaFree are unacceptable because they synchronise the whole device and
+ * stall the other streams.  For them the field buffer the x,y pass hands to the z pass (3 N floats) lives in a
+ * fixed array inside libdisc.so instead of in a context.
+ *
+ *   dims          (nx, ny, nz), each >= 1, HOST.  nx*ny*nz must not exceed DISC_NOALLOC_MAX_VOXELS (the size of the
+ *                 built-in array); a larger volume is rejected with DISC_ERR_INVALID_ARG and a message that names both
+ *                 numbers -- use a context and disc_smooth_field for it.
+ *   sigma_smooth  Gaussian sigma in voxels, > 0, ceil(3 sigma) <= DISC_MAX_GAUSS_RADIUS (else DISC_ERR_UNSUPPORTED).
+ *   disp_inout    DEVICE, 3*nx*ny*nz floats, planar, owned by the caller, updated in place.
+ *   stream        cudaStream_t of the CURRENT device; the call only enqueues two kernels on it and returns.
+ *
+ * Cost: the array is 3 * DISC_NOALLOC_MAX_VOXELS floats = 12 MiB of device memory, and every GPU on which this
+ * library gets loaded keeps that much reserved until the process exits, whether or not this function is ever called.
+ * First call on a device: it looks up the array's device address (cudaGetSymbolAddress), the device's compute
+ * capability and SM count, and keeps them; that is host-side set-up, not an allocation, but it talks to the driver, so
+ * make the first call on each device during start-up, before any stream capture is begun.  Later calls do no set-up.
+ * Sharing: there is ONE array per device and every call on that device uses it.  Two calls whose kernels may overlap
+ * on the GPU (different streams without an ordering between them, or two host threads) race on it and both results
+ * are undefined; calls on one stream, or ordered by events, are fine.  The array keeps whatever the last call left in
+ * it; nothing in it has to start at zero, because the x,y pass writes all 3 N floats before the z pass reads them.
+ * Errors go to disc_last_error(NULL) of the calling thread.  This function calls no cudaMalloc, no cudaFree and no
+ * library routine that allocates.
+ */
+#define DISC_NOALLOC_MAX_VOXELS (1 << 20) /* 128 x 128 x 64, config 2's finest level */
+disc_status disc_smooth_field_noalloc(const int dims[3], float sigma_smooth, float* disp_inout, void* stream);
 
 #ifdef __cplusplus
 }

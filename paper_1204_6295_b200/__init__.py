@@ -21,11 +21,13 @@ DISC_MAX_GAUSS_RADIUS = 12
 DISC_EPS_VAR = 1e-6
 DISC_EPS_DEN = 1e-3
 DISC_FORCE_THIRION, DISC_FORCE_DOUBLE = 1, 2
+DISC_NOALLOC_MAX_VOXELS = 1 << 20
 
 EXPORTS = (
     "disc_create", "disc_create_ex", "disc_destroy", "disc_last_error", "disc_launch_count", "disc_set_force", "disc_set_stop", "disc_iterations_run", "disc_set_mask", "disc_mask_params", "disc_get_ab", "disc_set_diagnostics", "disc_get_diagnostics", "disc_warp", "disc_correct_intensity",
     "disc_demons_step", "disc_register", "disc_register_host", "disc_iterate", "disc_box_moments",
     "disc_force_update", "disc_smooth_field", "disc_downsample", "disc_upsample_field", "disc_profile_iteration",
+    "disc_smooth_field_noalloc",
 )
 
 if not os.path.exists(LIB_PATH):
@@ -77,6 +79,8 @@ _lib.disc_iterate.restype = _i
 _lib.disc_iterate.argtypes = [_vp, _i, _vp, _vp, _vp, _i, _vp]
 _lib.disc_profile_iteration.restype = _i
 _lib.disc_profile_iteration.argtypes = [_vp, _i, _vp, _vp, _vp, _i, ctypes.POINTER(ctypes.c_float), _vp]
+_lib.disc_smooth_field_noalloc.restype = _i
+_lib.disc_smooth_field_noalloc.argtypes = [ctypes.POINTER(_i), ctypes.c_float, _vp, _vp]
 
 
 class DiscError(RuntimeError):
@@ -315,3 +319,14 @@ def disc_downsample(ctx, level_from, vol, out, stream=None):
 def disc_upsample_field(ctx, level_from, disp, out, stream=None):
     _check(ctx.handle, _lib.disc_upsample_field(ctx.handle, level_from, _dev(disp, _x3(ctx.n(level_from))),
                                                 _dev(out, _x3(ctx.n(level_from - 1))), _stream(stream)))
+
+
+def disc_smooth_field_noalloc(dims, sigma_smooth, disp_inout, stream=None):
+    """disc_smooth_field for callers that must not allocate device memory (an application that owns the GPU's memory
+    pool, or a latency-bound loop that cannot afford the device-wide stall of cudaMalloc): no context, the buffer
+    between the two kernels is a fixed 12 MiB array inside libdisc.so.  dims = (nx, ny, nz) with at most
+    DISC_NOALLOC_MAX_VOXELS voxels (more raises DiscError); calls that may overlap on the GPU race on that array;
+    make the first call on a device at start-up (it looks the array's address up).  See include/disc.h."""
+    d = (_i * 3)(*[int(v) for v in dims])
+    n = int(dims[0]) * int(dims[1]) * int(dims[2])
+    _check(None, _lib.disc_smooth_field_noalloc(d, float(sigma_smooth), _dev(disp_inout, 3 * n), _stream(stream)))

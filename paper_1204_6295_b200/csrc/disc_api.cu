@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "../../include/disc.h"
@@ -718,3 +719,87 @@ disc_status disc_upsample_field(disc_ctx* c, int level_from, const float* disp, 
 }
 
 }  // extern "C"
+
+// =====================================================================================
+// disc_smooth_field_noalloc: Gaussian regularisation for callers that may not allocate device memory (include/disc.h).
+// The buffer between the x,y pass and the z pass is this fixed array instead of a context's cudaMalloc'ed scratch.
+// In HOST code the name below is only a handle for cudaGetSymbolAddress: it is not a device address and must never be
+// handed to a kernel; the launches get the address looked up once per device in noalloc_device().
+static __device__ __align__(256) float g_noalloc_scratch[3 * (size_t)DISC_NOALLOC_MAX_VOXELS];
+
+namespace {
+
+struct NoAllocDev {
+    bool ready;
+    float* scratch;   // device address of g_noalloc_scratch on this device
+    DevInfo di;
+};
+NoAllocDev g_noalloc_dev[kMaxDevices];   // zero-initialised; guarded by g_noalloc_mutex
+std::mutex g_noalloc_mutex;
+
+// Per-device set-up, done by the first call on the current device: no allocation, only queries.
+disc_status noalloc_device(const NoAllocDev** out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(nullptr, DISC_ERR_CUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+    if (dev < 0 || dev >= kMaxDevices) return fail(nullptr, DISC_ERR_UNSUPPORTED, "device ordinal %d >= %d", dev, kMaxDevices);
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    NoAllocDev& d = g_noalloc_dev[dev];
+    if (!d.ready) {
+        int major = 0, n_sm = 0;
+        e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return fail(nullptr, DISC_ERR_CUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e));
+        if (major != 10) return fail(nullptr, DISC_ERR_UNSUPPORTED, "device compute capability %d.x, this library is sm_100a only", major);
+        float* p = nullptr;
+        e = cudaGetSymbolAddress((void**)&p, g_noalloc_scratch);   // the array's address on the CURRENT device
+        if (e != cudaSuccess || !p)
+            return fail(nullptr, DISC_ERR_CUDA, "cudaGetSymbolAddress(built-in scratch) on device %d: %s", dev, cudaGetErrorString(e));
+        d.scratch = p;
+        d.di.dev = dev;
+        d.di.n_sm = n_sm;
+        d.ready = true;
+    }
+    *out = &d;
+    return DISC_OK;
+}
+
+}  // namespace
+
+extern "C" disc_status disc_smooth_field_noalloc(const int dims[3], float sigma_smooth, float* disp_inout, void* stream) {
+    if (!dims || !disp_inout) return fail(nullptr, DISC_ERR_INVALID_ARG, "dims or disp_inout is NULL");
+    for (int i = 0; i < 3; ++i)
+        if (dims[i] < 1) return fail(nullptr, DISC_ERR_INVALID_ARG, "dims[%d] < 1", i);
+    const unsigned long long N = (unsigned long long)dims[0] * (unsigned long long)dims[1] * (unsigned long long)dims[2];
+    if ((unsigned long long)dims[0] * dims[1] > (unsigned long long)DISC_NOALLOC_MAX_VOXELS || N > (unsigned long long)DISC_NOALLOC_MAX_VOXELS)
+        return fail(nullptr, DISC_ERR_INVALID_ARG,
+                    "%d x %d x %d voxels exceed the built-in scratch of disc_smooth_field_noalloc (DISC_NOALLOC_MAX_VOXELS = %d): "
+                    "use a context and disc_smooth_field", dims[0], dims[1], dims[2], (int)DISC_NOALLOC_MAX_VOXELS);
+    if (!(sigma_smooth > 0.f)) return fail(nullptr, DISC_ERR_INVALID_ARG, "sigma_smooth <= 0");
+    const int K = (int)std::ceil(3.0 * (double)sigma_smooth);
+    if (K > DISC_MAX_GAUSS_RADIUS)
+        return fail(nullptr, DISC_ERR_UNSUPPORTED, "Gaussian radius ceil(3 sigma) = %d > %d", K, DISC_MAX_GAUSS_RADIUS);
+    const NoAllocDev* d = nullptr;
+    DISC_TRY(noalloc_device(&d));
+    // taps exactly as disc_create forms them: fp64, normalised to sum 1, then rounded to fp32 (reading A10)
+    GaussTaps taps;
+    std::memset(&taps, 0, sizeof(taps));
+    {
+        double w[kMaxGaussTaps], sum = 0.0;
+        for (int i = -K; i <= K; ++i) { w[i + K] = std::exp(-(double)(i * i) / (2.0 * (double)sigma_smooth * (double)sigma_smooth)); sum += w[i + K]; }
+        for (int i = 0; i < 2 * K + 1; ++i) taps.w[i] = (float)(w[i] / sum);
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const StopReq no_stop = {nullptr, 0, 0.f};
+    // x,y passes: disp_inout -> built-in array (all 3 N floats written); z pass: built-in array -> disp_inout
+    if (!launch_force_gxy_any(d->di, K, 0, nullptr, nullptr, disp_inout, d->scratch, dims[0], dims[1], dims[2], DISC_EPS_DEN, taps,
+                              kNoCtl, no_stop, st))
+        return fail(nullptr, DISC_ERR_UNSUPPORTED, "Gaussian radius %d unsupported", K);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(nullptr, DISC_ERR_CUDA, "k_force_gxy (no-alloc): %s", cudaGetErrorString(e));
+    if (!launch_gz_warp_any(d->di, K, false, d->scratch, disp_inout, nullptr, nullptr, dims[0], dims[1], dims[2], taps, kNoCtl, st))
+        return fail(nullptr, DISC_ERR_UNSUPPORTED, "Gaussian radius %d unsupported", K);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(nullptr, DISC_ERR_CUDA, "k_gz_warp (no-alloc): %s", cudaGetErrorString(e));
+    return DISC_OK;
+}
