@@ -152,13 +152,16 @@ disc_status disc_set_mask(disc_ctx* ctx, int enable, float hu0, float a_min, flo
  * later fine-grained calls: out_host = {Delta HU, HU_0, a_m, a_min, a_max} (HOST, 5 floats).  SYNCHRONISES `stream`. */
 disc_status disc_mask_params(disc_ctx* ctx, const float* ct, const float* cbct, float out_host[5], void* stream);
 
-/* a(x), b(x) and the mask of `level` as the last correction left them (device buffers, each may be NULL): out_a, out_b
- * [N_level] floats, out_xi [N_level] bytes -- 0: xi = 0, k in 1..254: xi = 1, filled in pass k, 255: xi = 1, never filled. */
+/* a(x), b(x) and the mask of `level` as the last correction left them -- after an early stop (disc_set_stop) those of the
+ * last iteration run -- (device buffers, each may be NULL): out_a, out_b [N_level] floats, out_xi [N_level] bytes --
+ * 0: xi = 0, k in 1..254: xi = 1, filled in pass k, 255: xi = 1, never filled. */
 disc_status disc_get_ab(disc_ctx* ctx, int level, float* out_a, float* out_b, unsigned char* out_xi, void* stream);
 
 /* Fig. 9 (e), (f) of the paper: the averages of a and of b over all voxels in every iteration of
  * disc_register.  disc_get_diagnostics SYNCHRONISES the device and writes levels*iters doubles each (HOST), level-major
- * from the COARSEST level, `iters` slots per level.  Without the mask this costs one more moments launch per iteration. */
+ * from the COARSEST level, `iters` slots per level; the slot of an iteration the last disc_register / disc_iterate did not
+ * run (stopping criterion tripped earlier, other level) reads NaN.  Without the mask this costs one more moments launch
+ * per iteration. */
 disc_status disc_set_diagnostics(disc_ctx* ctx, int enable);
 disc_status disc_get_diagnostics(disc_ctx* ctx, double* mean_a_host, double* mean_b_host);
 

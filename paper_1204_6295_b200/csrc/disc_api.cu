@@ -175,6 +175,28 @@ disc_status launch_upsample(disc_ctx* c, const Level& coarse, const float* in, f
 // ---------------------------------------------------------------- NEXT-1 plumbing
 bool ab_path(const disc_ctx* c) { return c->mask_on || c->diag_on; }
 
+// Fig.-9 slots of iterations that a run does not reach (early stop, disc_iterate on one level) read NaN, not the
+// previous run's averages: all-ones bytes are a quiet NaN in fp64.
+disc_status clear_diagnostics(disc_ctx* c, cudaStream_t st) {
+    if (!c->diag_on || !c->d_mean_a) return DISC_OK;
+    const size_t nd = (size_t)c->levels * (c->iters > 0 ? c->iters : 1) * sizeof(double);
+    if (cudaMemsetAsync(c->d_mean_a, 0xff, nd, st) != cudaSuccess || cudaMemsetAsync(c->d_mean_b, 0xff, nd, st) != cudaSuccess)
+        return fail(c, DISC_ERR_CUDA, "cudaMemsetAsync (diagnostics) failed");
+    return DISC_OK;
+}
+
+// frees the mask / diagnostics buffers and nulls the pointers (so that a later alloc_ab starts from scratch)
+void free_ab(disc_ctx* c) {
+    for (int l = 0; l < DISC_MAX_LEVELS; ++l) {
+        Level& L = c->lv[l];
+        cudaFree(L.mu_s); cudaFree(L.var_s); cudaFree(L.A); cudaFree(L.B); cudaFree(L.xi);
+        L.mu_s = L.var_s = L.A = L.B = nullptr; L.xi = nullptr;
+    }
+    cudaFree(c->d_mask); cudaFree(c->d_partial); cudaFree(c->d_mean_a); cudaFree(c->d_mean_b); cudaFree(c->cbct_shift);
+    c->d_mask = nullptr; c->d_partial = nullptr; c->d_mean_a = c->d_mean_b = nullptr; c->cbct_shift = nullptr;
+}
+
+// all or nothing: c->d_mask != NULL means every buffer below exists
 disc_status alloc_ab(disc_ctx* c) {
     if (c->d_mask) return DISC_OK;
     bool ok = cudaMalloc(&c->d_mask, sizeof(MaskCtl)) == cudaSuccess && cudaMemset(c->d_mask, 0, sizeof(MaskCtl)) == cudaSuccess &&
@@ -189,7 +211,11 @@ disc_status alloc_ab(disc_ctx* c) {
         ok = cudaMalloc(&L.mu_s, b) == cudaSuccess && cudaMalloc(&L.var_s, b) == cudaSuccess && cudaMalloc(&L.A, b) == cudaSuccess &&
              cudaMalloc(&L.B, b) == cudaSuccess && cudaMalloc(&L.xi, L.N) == cudaSuccess;
     }
-    if (!ok) { cudaGetLastError(); return fail(c, DISC_ERR_ALLOC, "cudaMalloc failed (mask / diagnostics buffers)"); }
+    if (!ok) {
+        cudaGetLastError();
+        free_ab(c);   // a retry must not find d_mask set with the other buffers missing
+        return fail(c, DISC_ERR_ALLOC, "cudaMalloc failed (mask / diagnostics buffers)");
+    }
     return DISC_OK;
 }
 
@@ -210,18 +236,18 @@ disc_status correct_ab(disc_ctx* c, const Level& L, const float* cbct, const flo
     DISC_TRY(launch_moments<kModeMoments>(c, L, m, nullptr, L.A, L.B, ctl, st));
     const unsigned g = reduce_grid(L.N);
     if (use_mask) {
-        k_fill_reset<<<1, 1, 0, st>>>(c->d_mask);
+        k_fill_reset<<<1, 1, 0, st>>>(c->d_mask, ctl);
         DISC_TRY(check_launch(c, "k_fill_reset"));
-        k_ab_mask<true><<<g, 256, 0, st>>>(m, cbct, L.mu_s, L.var_s, L.A, L.B, L.xi, L.N, DISC_EPS_VAR, c->d_mask);
+        k_ab_mask<true><<<g, 256, 0, st>>>(m, cbct, L.mu_s, L.var_s, L.A, L.B, L.xi, L.N, DISC_EPS_VAR, c->d_mask, ctl);
         DISC_TRY(check_launch(c, "k_ab_mask"));
         dim3 grid((L.nx + 127) / 128, L.ny, L.nz);
         const float inv_h2 = 1.f / (c->fill_h * c->fill_h);
         for (int p = 1; p <= c->max_fill_passes; ++p) {
-            k_fill_pass<<<grid, 128, 0, st>>>(cbct, L.A, L.B, L.xi, L.nx, L.ny, L.nz, c->fill_radius, inv_h2, p, c->d_mask);
+            k_fill_pass<<<grid, 128, 0, st>>>(cbct, L.A, L.B, L.xi, L.nx, L.ny, L.nz, c->fill_radius, inv_h2, p, c->d_mask, ctl);
             DISC_TRY(check_launch(c, "k_fill_pass"));
         }
     } else {
-        k_ab_mask<false><<<g, 256, 0, st>>>(m, cbct, L.mu_s, L.var_s, L.A, L.B, nullptr, L.N, DISC_EPS_VAR, c->d_mask);
+        k_ab_mask<false><<<g, 256, 0, st>>>(m, cbct, L.mu_s, L.var_s, L.A, L.B, nullptr, L.N, DISC_EPS_VAR, c->d_mask, ctl);
         DISC_TRY(check_launch(c, "k_ab"));
     }
     k_apply_ab<<<g, 256, 0, st>>>(cbct, L.A, L.B, out, L.N, c->d_partial, c->d_mask, slot >= 0 ? c->d_mean_a : nullptr,
@@ -556,6 +582,7 @@ disc_status disc_iterate(disc_ctx* c, int level, const float* ct, const float* c
     for (int l = 0; l < DISC_MAX_LEVELS; ++l) c->runs_host[l] = 0;
     if (c->stop_eps >= 0.f && cudaMemsetAsync(c->d_stop->runs, 0, sizeof(c->d_stop->runs), st) != cudaSuccess)
         return fail(c, DISC_ERR_CUDA, "cudaMemsetAsync failed");
+    DISC_TRY(clear_diagnostics(c, st));
     if (!c->mask_on) DISC_TRY(launch_moments<kModeZscore>(c, L, cbct, nullptr, L.zhat, nullptr, kNoCtl, st));
     if (ab_path(c)) DISC_TRY(cache_cbct_moments(c, L, cbct, st));
     DISC_TRY(launch_warp(c, L, ct, disp_inout, L.m, st));
@@ -614,6 +641,7 @@ disc_status disc_register(disc_ctx* c, const float* ct, const float* cbct, float
     const float* pct[DISC_MAX_LEVELS];
     const float* pcb[DISC_MAX_LEVELS];
     pct[0] = ct; pcb[0] = cbct;
+    DISC_TRY(clear_diagnostics(c, st));
     if (c->mask_on) {
         // A1 "Globally adjust the intensity of CBCT" and the mask parameters
         DISC_TRY(mask_parameters(c, ct, cbct, st));

@@ -92,7 +92,8 @@ template <bool USE_MASK>
 __global__ void __launch_bounds__(256)
 k_ab_mask(const float* __restrict__ m, const float* __restrict__ cbct, const float* __restrict__ mu_s,
           const float* __restrict__ var_s, float* __restrict__ A, float* __restrict__ B, unsigned char* __restrict__ xi,
-          size_t N, float eps_var, MaskCtl* ctl) {
+          size_t N, float eps_var, MaskCtl* ctl, IterCtl ictl) {
+    if (iter_skipped(ictl)) return;   // after an early stop A, B already hold a, b (not E(M), VAR(M)): leave them
     const float hu0 = ctl->hu0, a_min = ctl->a_min, a_max = ctl->a_max;
     unsigned masked = 0;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
@@ -173,7 +174,8 @@ static __global__ void k_select_step(int pass, MaskCtl* ctl) {
 // filled nothing, the remaining passes fall through.
 static __global__ void __launch_bounds__(128)
 k_fill_pass(const float* __restrict__ cbct, float* __restrict__ A, float* __restrict__ B, unsigned char* __restrict__ xi,
-            int nx, int ny, int nz, int rt, float inv_h2, int pass, MaskCtl* ctl) {
+            int nx, int ny, int nz, int rt, float inv_h2, int pass, MaskCtl* ctl, IterCtl ictl) {
+    if (iter_skipped(ictl)) return;
     {
         const volatile MaskCtl* c = ctl;
         if (c->remaining == 0u || (pass > 1 && c->prev_filled == 0u)) return;
@@ -244,7 +246,8 @@ k_fill_pass(const float* __restrict__ cbct, float* __restrict__ A, float* __rest
     }
 }
 
-static __global__ void k_fill_reset(MaskCtl* ctl) {
+static __global__ void k_fill_reset(MaskCtl* ctl, IterCtl ictl) {
+    if (iter_skipped(ictl)) return;
     ctl->remaining = 0u; ctl->filled = 0u; ctl->prev_filled = 0u; ctl->ticket = 0u;
 }
 

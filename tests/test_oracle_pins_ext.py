@@ -335,6 +335,27 @@ def test_register_ex_mask_composition_and_limits(oracle_mod):
     assert np.abs(o_on["disp"] - o_off["disp"]).max() < 1e-4
 
 
+@pytest.mark.parametrize("levels,auto", [(1, False), (2, True)])
+def test_stepwise_mask_chain_is_register_ex(oracle_mod, levels, auto):
+    """tests/next1_chain.py (Alg. A1 with the mask, one oracle call per step -- what the GPU parity test drives with the
+    CUDA path's Eq. (7) decisions) is, with its own decisions, bit for bit oracle.register_ex(mask=True)"""
+    import next1_chain
+    ct, cbct, _, _ = phantoms.make_pair(1, dims=(32, 24, 16))
+    R, sigma, iters, rt, h = 2, 1.5, 5, 2, 60.0
+    kw = {} if auto else dict(hu0=180.0, a_range=(0.5, 1.7))
+    o = oracle_mod.register_ex(ct, cbct, R, sigma, levels, iters, mask=True, fill_radius=rt, h=h, **kw)
+    seen = []
+    c = next1_chain.run(oracle_mod, ct, cbct, R, sigma, levels, iters, rt, h, decide=lambda l, k, m, s, a0, xi: (seen.append((l, k, xi.mean())), xi)[1], **kw)
+    assert np.array_equal(c["disp"], o["disp"]) and np.array_equal(c["corr"], o["corr"])
+    assert c["params"] == (o["info"]["hu0"], o["info"]["a_min"], o["info"]["a_max"])
+    assert [lk[:2] for lk in seen] == [(l, k) for l in range(levels - 1, -1, -1) for k in range(iters)] + [(0, iters)]
+    assert 0.0 < min(f for _, _, f in seen) and max(f for _, _, f in seen) < 1.0     # the mask fires, and not everywhere
+    # decisions matter: flipping them all gives another registration (so a test that overrides them does test something)
+    c2 = next1_chain.run(oracle_mod, ct, cbct, R, sigma, levels, 2, rt, h, decide=lambda l, k, m, s, a0, xi: ~xi, **kw)
+    c3 = next1_chain.run(oracle_mod, ct, cbct, R, sigma, levels, 2, rt, h, **kw)
+    assert np.abs(c2["disp"] - c3["disp"]).max() > 1e-3
+
+
 def test_mask_bounds_the_noise_free_case(oracle_mod):
     """Why the paper masks a: on a NOISE-FREE CBCT, flat regions have sigma_s ~ 0 and a = sigma_m /
     sigma_s explodes; the unmasked loop then drifts (DESIGN.md findings).  With Eq. (7) and the
