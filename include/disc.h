@@ -141,7 +141,9 @@ disc_status disc_set_stop(disc_ctx* ctx, float eps);
  *                   normalised by the largest one (same quotient, no underflow); passes stop when nothing is left, when a
  *                   pass fills nothing or after max_fill_passes, and what is then still unfilled keeps a = b = 0.
  * Everything is decided on the device (parameters, "anything left"): the iteration gets no host synchronisation.
- * disc_set_mask itself allocates 4 N floats + N bytes per level on first use and copies the given parameters to the
+ * The passes of one correction run in ONE cooperative launch over a compacted list of the xi = 1 voxels (grid barrier between
+ * passes), so a correction with few masked voxels costs little more than the unmasked one.
+ * disc_set_mask itself allocates 5 N words + N bytes per level on first use and copies the given parameters to the
  * device (a blocking cudaMemcpy of a few bytes); until disc_mask_params or disc_register has derived them, a parameter
  * given as < 0 reads HU_0 = 0, a_min = 0.5, a_max = 1.5.  enable == 0 switches back.
  */

@@ -34,6 +34,7 @@ struct Level {
     float* A;        // a(x): E(M) while it is being computed                            [N]
     float* B;        // b(x): VAR(M) while it is being computed                          [N]
     unsigned char* xi;  // 0 free, 255 masked and unfilled, k = filled in pass k         [N bytes]
+    unsigned* fill_list;  // voxel indices with xi = 1 of the running correction (N < 2^32)  [N]
 };
 
 thread_local char g_create_error[256] = "";
@@ -62,6 +63,7 @@ struct disc_ctx {
     float fill_h;
     int diag_on;      // Fig. 9 (e), (f): mean a, mean b per iteration
     MaskCtl* d_mask;
+    int fill_grid;       // blocks of k_fill_list (all resident: it is a cooperative launch)
     double* d_partial;   // block partials of the deterministic reductions   [2 * kReduceBlocks]
     double* d_mean_a;    // [levels * iters], level-major from the coarsest level
     double* d_mean_b;
@@ -189,8 +191,8 @@ disc_status clear_diagnostics(disc_ctx* c, cudaStream_t st) {
 void free_ab(disc_ctx* c) {
     for (int l = 0; l < DISC_MAX_LEVELS; ++l) {
         Level& L = c->lv[l];
-        cudaFree(L.mu_s); cudaFree(L.var_s); cudaFree(L.A); cudaFree(L.B); cudaFree(L.xi);
-        L.mu_s = L.var_s = L.A = L.B = nullptr; L.xi = nullptr;
+        cudaFree(L.mu_s); cudaFree(L.var_s); cudaFree(L.A); cudaFree(L.B); cudaFree(L.xi); cudaFree(L.fill_list);
+        L.mu_s = L.var_s = L.A = L.B = nullptr; L.xi = nullptr; L.fill_list = nullptr;
     }
     cudaFree(c->d_mask); cudaFree(c->d_partial); cudaFree(c->d_mean_a); cudaFree(c->d_mean_b); cudaFree(c->cbct_shift);
     c->d_mask = nullptr; c->d_partial = nullptr; c->d_mean_a = c->d_mean_b = nullptr; c->cbct_shift = nullptr;
@@ -210,6 +212,13 @@ disc_status alloc_ab(disc_ctx* c) {
         const size_t b = L.N * sizeof(float);
         ok = cudaMalloc(&L.mu_s, b) == cudaSuccess && cudaMalloc(&L.var_s, b) == cudaSuccess && cudaMalloc(&L.A, b) == cudaSuccess &&
              cudaMalloc(&L.B, b) == cudaSuccess && cudaMalloc(&L.xi, L.N) == cudaSuccess;
+        if (ok && L.N <= 0xffffffffull) ok = cudaMalloc(&L.fill_list, L.N * sizeof(unsigned)) == cudaSuccess;
+    }
+    // grid of the cooperative fill kernel: every block must be resident at once
+    if (ok) {
+        int per_sm = 0;
+        ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fill_list, 256, 0) == cudaSuccess && per_sm >= 1;
+        c->fill_grid = per_sm * c->di.n_sm;
     }
     if (!ok) {
         cudaGetLastError();
@@ -238,16 +247,28 @@ disc_status correct_ab(disc_ctx* c, const Level& L, const float* cbct, const flo
     if (use_mask) {
         k_fill_reset<<<1, 1, 0, st>>>(c->d_mask, ctl);
         DISC_TRY(check_launch(c, "k_fill_reset"));
-        k_ab_mask<true><<<g, 256, 0, st>>>(m, cbct, L.mu_s, L.var_s, L.A, L.B, L.xi, L.N, DISC_EPS_VAR, c->d_mask, ctl);
+        k_ab_mask<true><<<g, 256, 0, st>>>(m, cbct, L.mu_s, L.var_s, L.A, L.B, L.xi, L.N, DISC_EPS_VAR, c->d_mask, ctl, L.fill_list);
         DISC_TRY(check_launch(c, "k_ab_mask"));
-        dim3 grid((L.nx + 127) / 128, L.ny, L.nz);
         const float inv_h2 = 1.f / (c->fill_h * c->fill_h);
-        for (int p = 1; p <= c->max_fill_passes; ++p) {
-            k_fill_pass<<<grid, 128, 0, st>>>(cbct, L.A, L.B, L.xi, L.nx, L.ny, L.nz, c->fill_radius, inv_h2, p, c->d_mask, ctl);
-            DISC_TRY(check_launch(c, "k_fill_pass"));
+        if (L.fill_list) {
+            // all passes in one cooperative launch over the compacted list of masked voxels
+            const float* a_cbct = cbct; float* a_A = L.A; float* a_B = L.B; unsigned char* a_xi = L.xi;
+            const unsigned* a_list = L.fill_list;
+            int a_nx = L.nx, a_ny = L.ny, a_nz = L.nz, a_rt = c->fill_radius, a_max = c->max_fill_passes;
+            float a_h = inv_h2; MaskCtl* a_ctl = c->d_mask; IterCtl a_ictl = ctl;
+            void* args[] = {&a_cbct, &a_A, &a_B, &a_xi, &a_list, &a_nx, &a_ny, &a_nz, &a_rt, &a_h, &a_max, &a_ctl, &a_ictl};
+            cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_fill_list, dim3(c->fill_grid), dim3(256), args, 0, st);
+            if (e != cudaSuccess) return fail(c, DISC_ERR_CUDA, "k_fill_list: %s", cudaGetErrorString(e));
+            DISC_TRY(check_launch(c, "k_fill_list"));
+        } else {
+            dim3 grid((L.nx + 127) / 128, L.ny, L.nz);
+            for (int p = 1; p <= c->max_fill_passes; ++p) {
+                k_fill_pass<<<grid, 128, 0, st>>>(cbct, L.A, L.B, L.xi, L.nx, L.ny, L.nz, c->fill_radius, inv_h2, p, c->d_mask, ctl);
+                DISC_TRY(check_launch(c, "k_fill_pass"));
+            }
         }
     } else {
-        k_ab_mask<false><<<g, 256, 0, st>>>(m, cbct, L.mu_s, L.var_s, L.A, L.B, nullptr, L.N, DISC_EPS_VAR, c->d_mask, ctl);
+        k_ab_mask<false><<<g, 256, 0, st>>>(m, cbct, L.mu_s, L.var_s, L.A, L.B, nullptr, L.N, DISC_EPS_VAR, c->d_mask, ctl, nullptr);
         DISC_TRY(check_launch(c, "k_ab"));
     }
     k_apply_ab<<<g, 256, 0, st>>>(cbct, L.A, L.B, out, L.N, c->d_partial, c->d_mask, slot >= 0 ? c->d_mean_a : nullptr,

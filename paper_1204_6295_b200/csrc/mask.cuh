@@ -8,9 +8,12 @@
 //   k_shift           cbct + Delta HU  ("globally adjust the intensity of CBCT", Alg. A1)
 //   k_ab_mask         a = STD(M)/STD(S), b = E(M) - a E(S); xi by Eq. (7); a = b = 0 where xi = 1
 //   k_select_*        a_m = lower median of a over the voxels with both variances > eps (radix select)
-//   k_fill_pass       Eqs. (8)-(10), one Jacobi pass over the cube T
+//   k_fill_list       Eqs. (8)-(10): all Jacobi passes over the cube T in ONE cooperative launch, over the compacted
+//                     list of masked voxels that k_ab_mask wrote (grid barrier between passes)
+//   k_fill_pass       the same, one launch per pass over the whole volume (volumes of >= 2^32 voxels only)
 //   k_apply_ab        I'_s = a I_s + b, and the sums of a and b
 #pragma once
+#include <cooperative_groups.h>
 #include <float.h>
 
 #include "common.cuh"
@@ -31,6 +34,8 @@ struct MaskCtl {
     unsigned prefix;             // bits of the median fixed so far
     // fill passes
     unsigned remaining, filled, prev_filled, ticket;
+    unsigned n_list;             // masked voxels of the running correction (length of the compacted list)
+    unsigned filled_in[256];     // voxels filled by pass p (k_fill_list; slot 0 unused)
     // diagnostics of the running iteration
     double sum_a, sum_b;
     unsigned ticket2;
@@ -92,24 +97,38 @@ template <bool USE_MASK>
 __global__ void __launch_bounds__(256)
 k_ab_mask(const float* __restrict__ m, const float* __restrict__ cbct, const float* __restrict__ mu_s,
           const float* __restrict__ var_s, float* __restrict__ A, float* __restrict__ B, unsigned char* __restrict__ xi,
-          size_t N, float eps_var, MaskCtl* ctl, IterCtl ictl) {
+          size_t N, float eps_var, MaskCtl* ctl, IterCtl ictl, unsigned* __restrict__ list) {
     if (iter_skipped(ictl)) return;   // after an early stop A, B already hold a, b (not E(M), VAR(M)): leave them
     const float hu0 = ctl->hu0, a_min = ctl->a_min, a_max = ctl->a_max;
     unsigned masked = 0;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
-        const float mu_m = A[i], var_m = B[i], vs = __ldg(var_s + i);
-        const float a = vs > eps_var ? sqrtf(var_m / vs) : 0.f;          // Eq. (5); reading A5
-        const float b = fmaf(-a, __ldg(mu_s + i), mu_m);                 // Eq. (6)
+    // the loop bound is rounded up to whole warps: all 32 lanes of a warp reach the ballot below together
+    const size_t N32 = (N + 31) & ~(size_t)31;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N32; i += (size_t)gridDim.x * blockDim.x) {
         bool x = false;
-        if (USE_MASK) {
-            // Eq. (7): the difference of two fp32 values is taken in fp64 (exact), as is the comparison
-            const double d = fabs((double)__ldg(m + i) - (double)__ldg(cbct + i));
-            x = d > (double)hu0 || a < a_min || a > a_max;
+        if (i < N) {
+            const float mu_m = A[i], var_m = B[i], vs = __ldg(var_s + i);
+            const float a = vs > eps_var ? sqrtf(var_m / vs) : 0.f;          // Eq. (5); reading A5
+            const float b = fmaf(-a, __ldg(mu_s + i), mu_m);                 // Eq. (6)
+            if (USE_MASK) {
+                // Eq. (7): the difference of two fp32 values is taken in fp64 (exact), as is the comparison
+                const double d = fabs((double)__ldg(m + i) - (double)__ldg(cbct + i));
+                x = d > (double)hu0 || a < a_min || a > a_max;
+            }
+            A[i] = x ? 0.f : a;                                              // "Initially a = b = 0 for xi = 1"
+            B[i] = x ? 0.f : b;
+            if (xi) xi[i] = x ? kXiMasked : kXiFree;
+            masked += x ? 1u : 0u;
         }
-        A[i] = x ? 0.f : a;                                              // "Initially a = b = 0 for xi = 1"
-        B[i] = x ? 0.f : b;
-        if (xi) xi[i] = x ? kXiMasked : kXiFree;
-        masked += x ? 1u : 0u;
+        if (USE_MASK && list != nullptr) {
+            // compacted list of the masked voxels (the order is arbitrary and never matters: a fill pass treats every
+            // listed voxel independently); one atomic per warp
+            const unsigned vote = __ballot_sync(0xffffffffu, x);
+            const int lane = threadIdx.x & 31;
+            unsigned base = 0;
+            if (lane == 0 && vote) base = atomicAdd(&ctl->n_list, (unsigned)__popc(vote));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (x) list[base + __popc(vote & ((1u << lane) - 1u))] = (unsigned)i;
+        }
     }
     if (USE_MASK) {
         masked = __reduce_add_sync(0xffffffffu, masked);
@@ -246,9 +265,81 @@ k_fill_pass(const float* __restrict__ cbct, float* __restrict__ A, float* __rest
     }
 }
 
+// All passes in one cooperative launch over the compacted list (every block of the grid is resident; the grid barrier
+// separates the passes).  Same arithmetic, same order of the sums over T and same stamps as k_fill_pass.  A pass reads
+// a, b, xi only of voxels stamped before it started, i.e. written before the last grid barrier; what it writes is not
+// read until the next one.  filled_in[p] is written by pass p only and read after the barrier that ends it, so every
+// thread takes the same decision to go on or stop.  a, b, xi are read with plain (coherent) loads, never __ldg: they
+// change during the launch.
+static __global__ void __launch_bounds__(256)
+k_fill_list(const float* __restrict__ cbct, float* A, float* B, unsigned char* xi, const unsigned* __restrict__ list,
+            int nx, int ny, int nz, int rt, float inv_h2, int max_passes, MaskCtl* ctl, IterCtl ictl) {
+    if (iter_skipped(ictl)) return;                       // uniform over the grid: nobody reaches a barrier
+    const unsigned n = ctl->n_list;
+    if (n == 0u) return;                                  // idem
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    const unsigned stride = gridDim.x * blockDim.x;
+    unsigned remaining = n;
+    __shared__ unsigned blk;
+    for (int pass = 1; pass <= max_passes; ++pass) {
+        if (threadIdx.x == 0) blk = 0u;
+        __syncthreads();
+        unsigned mine = 0;
+        for (unsigned e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += stride) {
+            const unsigned i0 = list[e];
+            if (xi[i0] != kXiMasked) continue;
+            const int x = (int)(i0 % (unsigned)nx), y = (int)((i0 / (unsigned)nx) % (unsigned)ny), z = (int)(i0 / ((unsigned)nx * (unsigned)ny));
+            const float s0 = __ldg(cbct + i0);
+            const int xa = max(x - rt, 0), xb = min(x + rt, nx - 1);
+            const int ya = max(y - rt, 0), yb = min(y + rt, ny - 1);
+            const int za = max(z - rt, 0), zb = min(z + rt, nz - 1);
+            float dmin = FLT_MAX;
+            for (int c = za; c <= zb; ++c)
+                for (int b = ya; b <= yb; ++b) {
+                    const size_t row = ((size_t)c * ny + b) * nx;
+                    for (int a = xa; a <= xb; ++a) {
+                        if (xi[row + a] >= pass) continue;
+                        const float d = __ldg(cbct + row + a) - s0;
+                        dmin = fminf(dmin, d * d);
+                    }
+                }
+            if (dmin < FLT_MAX) {
+                float sw = 0.f, sa = 0.f, sb = 0.f;
+                for (int c = za; c <= zb; ++c)
+                    for (int b = ya; b <= yb; ++b) {
+                        const size_t row = ((size_t)c * ny + b) * nx;
+                        for (int a = xa; a <= xb; ++a) {
+                            if (xi[row + a] >= pass) continue;
+                            const float d = __ldg(cbct + row + a) - s0;
+                            const float w = __expf(-(d * d - dmin) * inv_h2);      // Eq. (10)
+                            sw += w;
+                            sa = fmaf(w, A[row + a], sa);
+                            sb = fmaf(w, B[row + a], sb);
+                        }
+                    }
+                A[i0] = sa / sw;                                                   // Eqs. (8), (9)
+                B[i0] = sb / sw;
+                xi[i0] = (unsigned char)pass;
+                ++mine;
+            }
+        }
+        mine = __reduce_add_sync(0xffffffffu, mine);
+        if ((threadIdx.x & 31) == 0 && mine) atomicAdd(&blk, mine);
+        __syncthreads();
+        if (threadIdx.x == 0 && blk) atomicAdd(&ctl->filled_in[pass], blk);
+        grid.sync();
+        const unsigned f = *reinterpret_cast<volatile unsigned*>(&ctl->filled_in[pass]);
+        remaining -= f;
+        if (f == 0u || remaining == 0u) break;            // nothing left, or a pass that filled nothing
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) ctl->remaining = remaining;
+}
+
 static __global__ void k_fill_reset(MaskCtl* ctl, IterCtl ictl) {
     if (iter_skipped(ictl)) return;
     ctl->remaining = 0u; ctl->filled = 0u; ctl->prev_filled = 0u; ctl->ticket = 0u;
+    ctl->n_list = 0u;
+    for (int p = 0; p < 256; ++p) ctl->filled_in[p] = 0u;
 }
 
 // ---------------------------------------------------------------- I'_s = a I_s + b and Fig. 9 (e), (f)
