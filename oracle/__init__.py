@@ -254,8 +254,12 @@ def box_moments3(vol, R, sat=False):
     v, pv = _f32(vol)
     mean = np.empty(v.shape, dtype=np.float64)
     var = np.empty(v.shape, dtype=np.float64)
-    fn = L.oracle_box_moments_sat if sat else L.oracle_box_moments3
-    fn(pv, *_dims(v), _r3(R), mean.ctypes.data_as(_f64p), var.ctypes.data_as(_f64p))
+    if sat:
+        L.oracle_box_moments_sat.restype = ctypes.c_int
+        if L.oracle_box_moments_sat(pv, *_dims(v), _r3(R), mean.ctypes.data_as(_f64p), var.ctypes.data_as(_f64p)) != 0:
+            raise ValueError("oracle_box_moments_sat: a value is not finite or |v| >= 2^14 HU (outside its fixed-point range)")
+    else:
+        L.oracle_box_moments3(pv, *_dims(v), _r3(R), mean.ctypes.data_as(_f64p), var.ctypes.data_as(_f64p))
     return mean, var
 
 

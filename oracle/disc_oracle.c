@@ -235,7 +235,8 @@ void oracle_force_norms(const float *m, const float *s, const float *disp, int n
     size_t N = (size_t)nx * ny * nz;
     float *tmp = (float *)calloc(3 * N, sizeof(float));
     double a = 0.0, b = 0.0;
-    /* the increment alone: the update applied to a zero field, in fp64 before the final rounding to fp32 */
+    /* the increment alone: the update applied to a zero field (evaluated in fp64, stored as the fp32 value that the
+     * update would add), summed in fp64 */
     if (double_force) oracle_force_update_double(m, s, nx, ny, nz, eps_den, tmp);
     else oracle_force_update(m, s, nx, ny, nz, eps_den, tmp);
     for (size_t i = 0; i < N; ++i) {
@@ -458,16 +459,17 @@ void oracle_box_moments3(const float *v, int nx, int ny, int nz, const int R[3],
  * inclusion-exclusion, and  n^2 var = n S2 - S1^2  (A.4) is formed exactly before the one conversion to
  * fp64 -- no cancellation error at all, which matters in flat regions: there sigma_m ~ 0 and an error of 1e-6 HU^2 in
  * the variance (what fp64 tables give on a 512x512x128 volume) becomes 1e-3 HU in the corrected image and, through the
- * demons force of a flat region, several 1e-3 voxel per iteration.  Returns without writing when a value is out of range. */
+ * demons force of a flat region, several 1e-3 voxel per iteration.  Returns 0; returns 1 WITHOUT writing mean and var
+ * when a value is not finite or |v| >= 2^14 HU (the fixed-point range): the caller must not use the outputs then. */
 typedef __int128 i128;
 
-void oracle_box_moments_sat(const float *v, int nx, int ny, int nz, const int R[3], double *mean, double *var) {
+int oracle_box_moments_sat(const float *v, int nx, int ny, int nz, const int R[3], double *mean, double *var) {
     const size_t N = (size_t)nx * ny * nz;
     const int px = nx + 1, py = ny + 1, pz = nz + 1;
     const size_t NP = (size_t)px * py * pz;
 #define PIDX(x, y, z) (((size_t)(z) * py + (y)) * px + (x))
     for (size_t i = 0; i < N; ++i)
-        if (!(fabsf(v[i]) < 16384.0f)) return;
+        if (!(fabsf(v[i]) < 16384.0f)) return 1;
     i128 *P1 = (i128 *)calloc(NP, sizeof(i128)), *P2 = (i128 *)calloc(NP, sizeof(i128));
     /* P[z+1][y+1][x+1] = sum over the box [0..x] x [0..y] x [0..z]; index 0 planes stay zero */
 #pragma omp parallel for schedule(static)
@@ -511,6 +513,7 @@ void oracle_box_moments_sat(const float *v, int nx, int ny, int nz, const int R[
             }
 #undef PIDX
     free(P1); free(P2);
+    return 0;
 }
 
 /* NEXT-4: pyramid with a per-axis factor f[c] in {1, 2} (the paper's own preprocessing halves only the transverse
@@ -705,8 +708,9 @@ static void level_dims(const oracle_params *p, int nx, int ny, int nz, int l, in
 
 static void moments_by_policy(const oracle_params *p, int k, int n_it, const float *v, int lx, int ly, int lz, double *mean,
                               double *var) {
-    if (p->moments_policy == 1 && k > 0 && k < n_it - 1) oracle_box_moments_sat(v, lx, ly, lz, p->R, mean, var);
-    else oracle_box_moments3(v, lx, ly, lz, p->R, mean, var);
+    /* the summed-area routine refuses values outside its fixed-point range: the naive loops take over */
+    if (p->moments_policy == 1 && k > 0 && k < n_it - 1 && oracle_box_moments_sat(v, lx, ly, lz, p->R, mean, var) == 0) return;
+    oracle_box_moments3(v, lx, ly, lz, p->R, mean, var);
 }
 
 /* A1 steps 1 (second half) to 3 from given patch moments: a, b by Eqs. (5)-(6); with the mask on, Eq. (7), the

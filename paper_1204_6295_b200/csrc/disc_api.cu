@@ -622,7 +622,12 @@ disc_status disc_profile_iteration(disc_ctx* c, int level, const float* ct, cons
     const int ne = 4 * n_iters;
     cudaEvent_t* ev = new (std::nothrow) cudaEvent_t[ne];
     if (!ev) return fail(c, DISC_ERR_ALLOC, "out of host memory");
-    for (int i = 0; i < ne; ++i) cudaEventCreate(&ev[i]);
+    for (int i = 0; i < ne; ++i)
+        if (cudaEventCreate(&ev[i]) != cudaSuccess) {
+            for (int j = 0; j < i; ++j) cudaEventDestroy(ev[j]);
+            delete[] ev;
+            return fail(c, DISC_ERR_CUDA, "cudaEventCreate failed: %s", cudaGetErrorString(cudaGetLastError()));
+        }
     disc_status rc = launch_moments<kModeZscore>(c, L, cbct, nullptr, L.zhat, nullptr, kNoCtl, st);
     if (rc == DISC_OK) rc = launch_warp(c, L, ct, disp_inout, L.m, st);
     for (int k = 0; k < n_iters && rc == DISC_OK; ++k) {

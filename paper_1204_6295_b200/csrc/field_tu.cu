@@ -30,8 +30,11 @@ static void launch_fg_t4s(const DevInfo& di, const float* m, const float* s, con
     using C = FgT4Cfg<K, TY>;
     static bool configured[kMaxDevices] = {};  // the opt-in is per device (idempotent, so a race is harmless)
     if (!configured[di.dev]) {
-        cudaFuncSetAttribute(k_force_gxy_t4<K, FORCE, TY, STOP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
-        configured[di.dev] = true;
+        // on failure the flag stays clear and the launch below fails with a shared-memory error that cudaGetLastError
+        // in the caller reports
+        if (cudaFuncSetAttribute(k_force_gxy_t4<K, FORCE, TY, STOP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)C::smem_bytes) == cudaSuccess)
+            configured[di.dev] = true;
     }
     const long long n_tiles = (long long)((nx + C::TX - 1) / C::TX) * ((ny + C::TY - 1) / C::TY) * nz;
     const int grid = (int)(n_tiles < (long long)C::OCC * di.n_sm ? n_tiles : (long long)C::OCC * di.n_sm);   // persistent: OCC CTAs per SM

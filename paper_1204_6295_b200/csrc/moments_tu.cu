@@ -79,8 +79,10 @@ static bool launch_r_v3(const DevInfo& di, int rz, int mode, const float* vol, c
 #define DISC_LAUNCH_MODE(M)                                                                                              \
     {                                                                                                                    \
         if (!configured[M][di.dev]) {   /* the opt-in is per device */                                                   \
-            cudaFuncSetAttribute(k_moments_v3<R, TY, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes); \
-            configured[M][di.dev] = true;                                                                                \
+            /* on failure the flag stays clear and the launch fails with an error the caller's cudaGetLastError reports */ \
+            if (cudaFuncSetAttribute(k_moments_v3<R, TY, M>, cudaFuncAttributeMaxDynamicSharedMemorySize,               \
+                                     (int)C::smem_bytes) == cudaSuccess)                                                 \
+                configured[M][di.dev] = true;                                                                            \
         }                                                                                                                \
         k_moments_v3<R, TY, M><<<grid, C::NT, C::smem_bytes, st>>>(tmap, pv, out0, out1, nx, ny, nz, rz, zchunk, eps_var, ctl); \
     }
@@ -127,8 +129,9 @@ static bool launch_r_blk(const DevInfo& di, int rz, int mode, const float* vol, 
 #define DISC_LAUNCH_MODE(M)                                                                                              \
     {                                                                                                                    \
         if (!configured[M][di.dev]) {   /* the opt-in is per device */                                                   \
-            cudaFuncSetAttribute(k_moments_blk<R, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);       \
-            configured[M][di.dev] = true;                                                                                \
+            if (cudaFuncSetAttribute(k_moments_blk<R, M>, cudaFuncAttributeMaxDynamicSharedMemorySize,                  \
+                                     (int)kSmemMax) == cudaSuccess)                                                      \
+                configured[M][di.dev] = true;                                                                            \
         }                                                                                                                \
         k_moments_blk<R, M><<<grid, C::NT, smem, st>>>(tmap, pv, out0, out1, nx, ny, nz, rz, by, bz, eps_var, ctl);      \
     }

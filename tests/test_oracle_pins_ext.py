@@ -97,6 +97,23 @@ def test_sat_moments_match_naive(oracle_mod, shape, R):
     np.testing.assert_allclose(vs, bv, rtol=0, atol=1e-8)
 
 
+def test_sat_moments_refuse_values_outside_their_range(oracle_mod):
+    """the fixed-point tables hold |v| < 2^14 HU: anything else is an error, not silently unwritten outputs; the driver
+    falls back to the naive loops (same result as without the policy)"""
+    v = np.zeros((4, 5, 6), dtype=np.float32)
+    for bad in (16384.0, -3e4, np.inf, np.nan):
+        v[1, 2, 3] = bad
+        with pytest.raises(ValueError):
+            oracle_mod.box_moments3(v, 1, sat=True)
+    rng = np.random.default_rng(5)
+    ct = rng.normal(0, 100, size=(8, 8, 8)).astype(np.float32)
+    cbct = ct + rng.normal(0, 20, size=ct.shape).astype(np.float32)
+    ct[0, 0, 0] = 20000.0
+    a = oracle_mod.register_ex(ct, cbct, 1, 1.0, 1, 4, sat_between=True)
+    b = oracle_mod.register_ex(ct, cbct, 1, 1.0, 1, 4)
+    assert np.array_equal(a["disp"], b["disp"])
+
+
 def test_sat_moments_on_a_phantom(oracle_mod):
     """HU-scale data with large flat regions: the summed-area route is exact integer arithmetic up to the one final
     conversion, so a flat patch has var = 0 EXACTLY (as in the naive two-pass loop) and everywhere else the two agree
