@@ -148,33 +148,106 @@ def run_reference(args):
 SWEEP_SIZES = ((64, 64, 64), (128, 128, 128), (256, 256, 256), (512, 512, 256))
 
 
-def run_sweep(args):
-    """--sweep: BASELINE.json configs[4] -- every exported kernel alone, on seeded smooth random volumes / fields, at
-    64^3 .. 512x512x256; achieved GB/s = algorithmic bytes / CUDA-event time, vs the HBM peak.
-    The working sets at 64^3 and 128^3 (and most of 256^3) fit the 126 MB L2: those rows are L2-resident numbers."""
+L2_BYTES = 126 * 1000 * 1000
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r03_traffic.csv")
+NCU_KERNELS = (("k_moments_v3", "moments_correct"), ("k_force_gxy_t4", "force_gauss_xy"), ("k_gz_warp_d2", "gauss_z_warp"))
+
+
+def kernel_source_hash():
+    from paper_1204_6295_b200 import build as _build
+    return _build._source_hash()
+
+
+def write_traffic(paths):
+    """--write-traffic a.csv,b.csv,...: each file is `ncu -i <rep> --page raw --csv --print-units base` of ONE launch of
+    one iteration kernel at the finest level of config 3; writes profiles/r03_traffic.csv (dram__bytes_read.sum +
+    dram__bytes_write.sum per launch) stamped with the hash of the kernel sources in the tree."""
+    import csv
+    out = {}
+    for path in paths.split(","):
+        rows = list(csv.reader(open(path)))
+        head = next(i for i, r in enumerate(rows) if "Kernel Name" in r)
+        cols = rows[head]
+        for r in rows[head + 2:]:                       # rows[head + 1] holds the units
+            if len(r) != len(cols):
+                continue
+            rec = dict(zip(cols, r))
+            for pat, key in NCU_KERNELS:
+                if pat in rec["Kernel Name"]:
+                    out[key] = int(float(rec["dram__bytes_read.sum"].replace(",", ""))) + \
+                               int(float(rec["dram__bytes_write.sum"].replace(",", "")))
+    missing = [k for _, k in NCU_KERNELS if k not in out]
+    if missing:
+        print(f"no launch of {missing} in {paths}", file=sys.stderr)
+        return 1
+    with open(TRAFFIC_CSV, "w") as f:
+        f.write("# ncu --set full --clock-control none, one finest-level launch per kernel at 256x256x128 "
+                "(profiles/r03_launches_and_ncu.md): dram__bytes_read.sum + dram__bytes_write.sum; "
+                f"kernel_sources_sha256={kernel_source_hash()}\n")
+        f.write("kernel,dram_bytes_per_launch\n")
+        for _, k in NCU_KERNELS:
+            f.write(f"{k},{out[k]}\n")
+    print(open(TRAFFIC_CSV).read())
+    return 0
+
+
+def read_traffic(kernel):
+    """(bytes per launch or None, where the figure comes from / why it is withheld)"""
+    if not os.path.exists(TRAFFIC_CSV):
+        return None, "no capture committed (profiles/r03_traffic.csv)"
+    try:
+        lines = open(TRAFFIC_CSV).read().splitlines()
+        source = lines[0].lstrip("# ").strip()
+        stamp = source.rsplit("kernel_sources_sha256=", 1)[1].strip()
+        if stamp != kernel_source_hash():
+            return None, "stale: the kernel sources changed after the capture in profiles/r03_traffic.csv was taken"
+        for ln in lines[2:]:
+            f = ln.split(",")
+            if f[0] == kernel:
+                return float(f[1]), source
+    except Exception as exc:                               # a malformed file is reported, not hidden
+        return None, f"unreadable profiles/r03_traffic.csv: {exc}"
+    return None, "kernel not in profiles/r03_traffic.csv"
+
+
+def sweep_rows(sizes, radii, sigmas, peak, n_timed=30):
+    """BASELINE.json configs[4]: every exported kernel alone on seeded smooth random volumes / fields
+    (phantoms.make_sweep_inputs).  One row per (kernel, size, parameter): `ms` = mean of n_timed back-to-back launches
+    (CUDA events on the launching stream), achieved GB/s = algorithmic bytes / ms, `frac` of the
+    measured HBM peak.  Rows whose working set fits the L2 are labelled "L2-resident" and carry a second, COLD timing
+    (`cold_ms`, `cold_gbs`, `cold_frac`): a 256 MiB memset between launches evicts the working set, each launch timed
+    by its own event pair."""
     import torch
 
     import paper_1204_6295_b200 as disc
     import phantoms
 
-    torch.cuda.set_device(0)
-    peak, peak_src = measured_peak_gbs()
     stream = torch.cuda.current_stream()
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
     rows = []
 
-    def timed(fn, n_warm=5, n=30):
+    def timed(fn, n_warm=5):
         for _ in range(n_warm):
             fn()
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
-        for _ in range(n):
+        for _ in range(n_timed):
             fn()
         e1.record(stream)
         torch.cuda.synchronize()
-        return e0.elapsed_time(e1) / n
+        return e0.elapsed_time(e1) / n_timed
 
-    sizes = SWEEP_SIZES[:args.sweep_max] if args.sweep_max else SWEEP_SIZES
+    def timed_cold(fn, n=10):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+        for e0, e1 in ev:
+            flush.zero_()
+            e0.record(stream)
+            fn()
+            e1.record(stream)
+        torch.cuda.synchronize()
+        return sum(e0.elapsed_time(e1) for e0, e1 in ev) / n
+
     for dims in sizes:
         nx, ny, nz = dims
         n = nx * ny * nz
@@ -184,28 +257,49 @@ def run_sweep(args):
         d_r = d_u.clone()
         tag = f"{nx}x{ny}x{nz}"
 
-        def add(kernel, param, bpv, ms):
+        def add(kernel, param, bpv, fn, resident_bytes):
+            ms = timed(fn)
             gbs = bpv * n / (ms * 1e-3) / 1e9
-            rows.append({"kernel": kernel, "size": tag, "param": param, "ms": ms, "bytes_per_voxel": bpv, "gbs": gbs,
-                         "frac": gbs / peak})
+            row = {"kernel": kernel, "size": tag, "param": param, "ms": ms, "bytes_per_voxel": bpv, "gbs": gbs,
+                   "frac": gbs / peak}
+            if resident_bytes * n <= L2_BYTES:
+                cms = timed_cold(fn)
+                cg = bpv * n / (cms * 1e-3) / 1e9
+                row.update({"cache": "L2-resident (warm, back to back)", "cold_ms": cms, "cold_gbs": cg, "cold_frac": cg / peak})
+            else:
+                row["cache"] = "exceeds L2"
+            rows.append(row)
 
+        # resident_bytes: bytes per voxel the call touches (inputs + outputs + context scratch)
         ctx = disc.disc_create(dims, (1.0, 1.0, 1.0), 1, 1.0, 1, 1)
-        add("disc_warp", None, 20.0, timed(lambda: disc.disc_warp(ctx, 0, d_a, d_u, d_o)))
-        add("disc_force_update", None, 32.0, timed(lambda: disc.disc_force_update(ctx, 0, d_a, d_b, d_r)))
+        add("disc_warp", None, 20.0, lambda: disc.disc_warp(ctx, 0, d_a, d_u, d_o), 20.0)
+        add("disc_force_update", None, 32.0, lambda: disc.disc_force_update(ctx, 0, d_a, d_b, d_r), 20.0)
         disc.disc_destroy(ctx)
-        for R in range(1, 11):
+        for R in radii:
             ctx = disc.disc_create(dims, (1.0, 1.0, 1.0), R, 1.0, 1, 1)
-            add("disc_box_moments", f"R={R}", 12.0, timed(lambda: disc.disc_box_moments(ctx, 0, d_a, d_o, d_o2)))
+            add("disc_box_moments", f"R={R}", 12.0, lambda: disc.disc_box_moments(ctx, 0, d_a, d_o, d_o2), 12.0)
             disc.disc_destroy(ctx)
-        for sigma in (1.0, 1.5, 2.0, 2.5, 3.0):
+        for sigma in sigmas:
             ctx = disc.disc_create(dims, (1.0, 1.0, 1.0), 1, sigma, 1, 1)
             d_r.copy_(d_u)
-            add("disc_smooth_field", f"sigma={sigma}", 24.0, timed(lambda: disc.disc_smooth_field(ctx, 0, d_r)))
+            add("disc_smooth_field", f"sigma={sigma}", 24.0, lambda: disc.disc_smooth_field(ctx, 0, d_r), 24.0)
             disc.disc_destroy(ctx)
         del d_a, d_b, d_u, d_o, d_o2, d_r
         torch.cuda.empty_cache()
+    return rows
+
+
+def run_sweep(args):
+    """--sweep: BASELINE.json configs[4], the full grid: R = 1..10, sigma = 1..3 in steps of 0.5, 64^3 .. 512x512x256."""
+    import torch
+
+    torch.cuda.set_device(0)
+    peak, peak_src = measured_peak_gbs()
+    sizes = SWEEP_SIZES[:args.sweep_max] if args.sweep_max > 0 else SWEEP_SIZES
+    rows = sweep_rows(sizes, range(1, 11), (1.0, 1.5, 2.0, 2.5, 3.0), peak)
     print(json.dumps({"sweep": "config5 per-kernel", "peak_gbs": peak, "peak_source": peak_src, "unit": "GB/s",
-                      "note": "64^3 and 128^3 working sets are L2-resident; 30 back-to-back launches per point", "rows": rows}))
+                      "note": "rows labelled L2-resident carry a warm (back-to-back) and a cold (256 MiB memset between "
+                              "launches) timing; 30 back-to-back launches per warm point, 10 per cold point", "rows": rows}))
     return 0
 
 
@@ -219,9 +313,14 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json config 5: per-kernel GB/s sweep (1 GPU)")
     ap.add_argument("--sweep-max", type=int, default=0, help="only the first n sizes of the sweep")
+    ap.add_argument("--no-sweep", action="store_true", help="leave the compact config-5 sweep out of the bench line")
+    ap.add_argument("--write-traffic", metavar="NCU_RAW_CSV", help="write profiles/r03_traffic.csv from `ncu -i <rep> --page "
+                    "raw --csv` output of one finest-level launch per iteration kernel, stamped with the hash of the kernel sources")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.write_traffic:
+        return write_traffic(args.write_traffic)
     if args.sweep:
         return run_sweep(args)
 
@@ -413,25 +512,28 @@ def main():
         per_kernel.append({"kernel": name, "ms": ms, "bytes_per_voxel": bpv, "gbs": gbs, "frac": gbs / peak})
     dom = max(per_kernel, key=lambda k: k["ms"])
     # DRAM bytes per launch are not measurable inside this run (no profiler here): they come from the committed
-    # `ncu --set full` capture of the SAME kernels, and the line says which capture and which commit it belongs to
-    traffic, traffic_source = None, None
-    tpath = os.path.join(ROOT, "profiles", "r02_traffic.csv")
-    if os.path.exists(tpath):
-        try:
-            lines = open(tpath).read().splitlines()
-            traffic_source = lines[0].lstrip("# ").strip()
-            for ln in lines[2:]:
-                f = ln.split(",")
-                if f[0] == dom["kernel"]:
-                    traffic = float(f[1])
-        except Exception:
-            traffic, traffic_source = None, None
+    # `ncu --set full` capture of the SAME kernels.  The capture is stamped with the hash of the kernel sources it was
+    # taken from; when the sources have changed since, the figure is stale and the line carries null instead.
+    traffic, traffic_source = read_traffic(dom["kernel"])
     roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["gbs"], "peak": peak, "unit": "GB/s",
                 "frac": dom["gbs"] / peak, "frac_of_nominal_8tbs": dom["gbs"] / 8000.0, "traffic": traffic,
                 "traffic_source": traffic_source, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": dom["bytes_per_voxel"] * n0, "per_kernel": per_kernel,
                 "iteration_bytes_per_voxel": ITER_BPV, "iteration_gbs": ITER_BPV * n0 / (ms_iter * 1e-3) / 1e9,
                 "iteration_frac": ITER_BPV * n0 / (ms_iter * 1e-3) / 1e9 / peak}
+
+    # ---------------- config 5 in the driver-run line: a compact per-kernel sweep (full grid: bench.py --sweep)
+    sweep = None
+    if world == 1 and not args.no_sweep:
+        disc.disc_destroy(ctx)
+        del d_ct, d_cb, d_r, d_corr, d_r2, u_true
+        torch.cuda.empty_cache()
+        sweep = {"sizes": ["x".join(map(str, d)) for d in SWEEP_SIZES], "radii": [1, 5, 10], "sigmas": [1.0, 2.0, 3.0],
+                 "unit": "GB/s", "peak_gbs": peak,
+                 "note": "algorithmic bytes / CUDA-event time; L2-resident rows also carry a cold timing (256 MiB memset "
+                         "between launches); full grid: python bench.py --sweep",
+                 "rows": sweep_rows(SWEEP_SIZES, (1, 5, 10), (1.0, 2.0, 3.0), peak, n_timed=20)}
+        ctx = None
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -460,10 +562,11 @@ def main():
                               "ms_per_registration": ms_clinical},
         "e2e": {"value": e2e_value, "unit": "voxel-updates/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": ms_e2e / n_e2e},
-        "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
+        "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu, "sweep": sweep,
     }
     print(json.dumps(line))
-    disc.disc_destroy(ctx)
+    if ctx is not None:
+        disc.disc_destroy(ctx)
     if dist is not None:
         dist.destroy_process_group()
     return 0

@@ -27,6 +27,52 @@ static EncodeTiledFn encode_tiled() {
     return fn;
 }
 
+// Tiled fp32 tensor map of an (nx, ny, nz) volume with a (bx, by, bz) box, out-of-volume elements read as zero.
+// A map encodes nothing but the base address, the shape and the box, so it can be reused whenever those recur -- in the
+// iteration loop the source is always the context's warped-CT buffer of the level, and cuTensorMapEncodeTiled per launch
+// was pure host overhead (the coarse levels are launch-bound).  Small per-thread cache, least recently used out.
+static bool tensor_map_3d(EncodeTiledFn enc, const float* vol, int nx, int ny, int nz, int bx, int by, int bz,
+                          CUtensorMap* out) {
+    struct Entry {
+        const float* vol;
+        int d[6];
+        unsigned long long used;
+        CUtensorMap map;
+    };
+    constexpr int kEntries = 16;
+    static thread_local Entry cache[kEntries] = {};
+    static thread_local unsigned long long tick = 0;
+    const int d[6] = {nx, ny, nz, bx, by, bz};
+    int victim = 0;
+    ++tick;
+    for (int i = 0; i < kEntries; ++i) {
+        Entry& e = cache[i];
+        if (e.used && e.vol == vol && e.d[0] == d[0] && e.d[1] == d[1] && e.d[2] == d[2] && e.d[3] == d[3] &&
+            e.d[4] == d[4] && e.d[5] == d[5]) {
+            e.used = tick;
+            *out = e.map;
+            return true;
+        }
+        if (e.used < cache[victim].used) victim = i;
+    }
+    const cuuint64_t gdim[3] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz};
+    const cuuint64_t gstr[2] = {(cuuint64_t)nx * 4, (cuuint64_t)nx * ny * 4};
+    const cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, (cuuint32_t)bz};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    Entry& e = cache[victim];
+    if (enc(&e.map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(vol), gdim, gstr, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
+        e.used = 0;
+        return false;
+    }
+    e.vol = vol;
+    for (int i = 0; i < 6; ++i) e.d[i] = d[i];
+    e.used = tick;
+    *out = e.map;
+    return true;
+}
+
 // the plain definition for everything the sliding-window kernels do not cover (moments.cuh)
 static void launch_moments_direct(int rx, int ry, int rz, int mode, const float* vol, const float* aux, float* out0,
                                   float* out1, int nx, int ny, int nz, float eps_var, IterCtl ctl, cudaStream_t st) {
@@ -62,14 +108,7 @@ static bool launch_r_v3(const DevInfo& di, int rz, int mode, const float* vol, c
     EncodeTiledFn enc = encode_tiled();
     if (!enc) return false;
     CUtensorMap tmap;
-    const cuuint64_t gdim[3] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz};
-    const cuuint64_t gstr[2] = {(cuuint64_t)nx * 4, (cuuint64_t)nx * ny * 4};
-    const cuuint32_t box[3] = {(cuuint32_t)C::PXB, (cuuint32_t)C::PY, 1};
-    const cuuint32_t estr[3] = {1, 1, 1};
-    if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(vol), gdim, gstr, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-        return false;
+    if (!tensor_map_3d(enc, vol, nx, ny, nz, C::PXB, C::PY, 1, &tmap)) return false;
     // per-voxel operand of the evaluation: the volume itself (z-score), the cached z-score (correction)
     const float* pv = mode == kModeCorrect ? aux : vol;
     const long long tiles = (long long)((nx + C::TX - 1) / C::TX) * ((ny + TY - 1) / TY);
@@ -114,14 +153,7 @@ static bool launch_r_blk(const DevInfo& di, int rz, int mode, const float* vol, 
     EncodeTiledFn enc = encode_tiled();
     if (!enc) return false;
     CUtensorMap tmap;
-    const cuuint64_t gdim[3] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz};
-    const cuuint64_t gstr[2] = {(cuuint64_t)nx * 4, (cuuint64_t)nx * ny * 4};
-    const cuuint32_t box[3] = {(cuuint32_t)C::PXB, (cuuint32_t)py, (cuuint32_t)pz};
-    const cuuint32_t estr[3] = {1, 1, 1};
-    if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(vol), gdim, gstr, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-        return false;
+    if (!tensor_map_3d(enc, vol, nx, ny, nz, C::PXB, py, pz, &tmap)) return false;
     const float* pv = mode == kModeCorrect ? aux : vol;
     dim3 grid((nx + C::TX - 1) / C::TX, (ny + by - 1) / by, (nz + bz - 1) / bz);
     const size_t smem = C::smem_bytes(py, pz);
