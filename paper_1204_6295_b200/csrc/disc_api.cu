@@ -34,7 +34,8 @@ struct Level {
     float* A;        // a(x): E(M) while it is being computed                            [N]
     float* B;        // b(x): VAR(M) while it is being computed                          [N]
     unsigned char* xi;  // 0 free, 255 masked and unfilled, k = filled in pass k         [N bytes]
-    unsigned* fill_list;  // voxel indices with xi = 1 of the running correction (N < 2^32)  [N]
+    unsigned* fill_list;  // work lists of the fill passes: odd passes [0, N), even passes [N, 2N)  (N < 2^32)  [2N]
+    unsigned* fill_queued;  // one bit per voxel: already on the next pass's list          [ceil(N/32)]
 };
 
 thread_local char g_create_error[256] = "";
@@ -177,6 +178,15 @@ disc_status launch_upsample(disc_ctx* c, const Level& coarse, const float* in, f
 // ---------------------------------------------------------------- NEXT-1 plumbing
 bool ab_path(const disc_ctx* c) { return c->mask_on || c->diag_on; }
 
+// grid of the cooperative fill kernel: every block must be resident at once
+disc_status fill_grid_for(disc_ctx* c, int* grid) {
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fill_list, 256, 0) != cudaSuccess || per_sm < 1)
+        return fail(c, DISC_ERR_CUDA, "no resident block of the fill kernel: %s", cudaGetErrorString(cudaGetLastError()));
+    *grid = per_sm * c->di.n_sm;
+    return DISC_OK;
+}
+
 // Fig.-9 slots of iterations that a run does not reach (early stop, disc_iterate on one level) read NaN, not the
 // previous run's averages: all-ones bytes are a quiet NaN in fp64.
 disc_status clear_diagnostics(disc_ctx* c, cudaStream_t st) {
@@ -191,8 +201,8 @@ disc_status clear_diagnostics(disc_ctx* c, cudaStream_t st) {
 void free_ab(disc_ctx* c) {
     for (int l = 0; l < DISC_MAX_LEVELS; ++l) {
         Level& L = c->lv[l];
-        cudaFree(L.mu_s); cudaFree(L.var_s); cudaFree(L.A); cudaFree(L.B); cudaFree(L.xi); cudaFree(L.fill_list);
-        L.mu_s = L.var_s = L.A = L.B = nullptr; L.xi = nullptr; L.fill_list = nullptr;
+        cudaFree(L.mu_s); cudaFree(L.var_s); cudaFree(L.A); cudaFree(L.B); cudaFree(L.xi); cudaFree(L.fill_list); cudaFree(L.fill_queued);
+        L.mu_s = L.var_s = L.A = L.B = nullptr; L.xi = nullptr; L.fill_list = nullptr; L.fill_queued = nullptr;
     }
     cudaFree(c->d_mask); cudaFree(c->d_partial); cudaFree(c->d_mean_a); cudaFree(c->d_mean_b); cudaFree(c->cbct_shift);
     c->d_mask = nullptr; c->d_partial = nullptr; c->d_mean_a = c->d_mean_b = nullptr; c->cbct_shift = nullptr;
@@ -212,13 +222,9 @@ disc_status alloc_ab(disc_ctx* c) {
         const size_t b = L.N * sizeof(float);
         ok = cudaMalloc(&L.mu_s, b) == cudaSuccess && cudaMalloc(&L.var_s, b) == cudaSuccess && cudaMalloc(&L.A, b) == cudaSuccess &&
              cudaMalloc(&L.B, b) == cudaSuccess && cudaMalloc(&L.xi, L.N) == cudaSuccess;
-        if (ok && L.N <= 0xffffffffull) ok = cudaMalloc(&L.fill_list, L.N * sizeof(unsigned)) == cudaSuccess;
-    }
-    // grid of the cooperative fill kernel: every block must be resident at once
-    if (ok) {
-        int per_sm = 0;
-        ok = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fill_list, 256, 0) == cudaSuccess && per_sm >= 1;
-        c->fill_grid = per_sm * c->di.n_sm;
+        if (ok && L.N <= 0xffffffffull)
+            ok = cudaMalloc(&L.fill_list, 2 * L.N * sizeof(unsigned)) == cudaSuccess &&
+                 cudaMalloc(&L.fill_queued, (L.N + 31) / 32 * sizeof(unsigned)) == cudaSuccess;
     }
     if (!ok) {
         cudaGetLastError();
@@ -247,16 +253,20 @@ disc_status correct_ab(disc_ctx* c, const Level& L, const float* cbct, const flo
     if (use_mask) {
         k_fill_reset<<<1, 1, 0, st>>>(c->d_mask, ctl);
         DISC_TRY(check_launch(c, "k_fill_reset"));
-        k_ab_mask<true><<<g, 256, 0, st>>>(m, cbct, L.mu_s, L.var_s, L.A, L.B, L.xi, L.N, DISC_EPS_VAR, c->d_mask, ctl, L.fill_list);
+        // one round per block (each round of the list append holds three block barriers: a grid-stride loop of 55 rounds
+        // ran them back to back, 157 us at 256x256x128; independent blocks overlap them)
+        const size_t nb = (L.N + 255) / 256;
+        const unsigned gm = (unsigned)(nb < 0x7fffffffull ? nb : 0x7fffffffull);
+        k_ab_mask<true><<<gm, 256, 0, st>>>(m, cbct, L.mu_s, L.var_s, L.A, L.B, L.xi, L.N, DISC_EPS_VAR, c->d_mask, ctl, L.fill_list, L.fill_queued);
         DISC_TRY(check_launch(c, "k_ab_mask"));
         const float inv_h2 = 1.f / (c->fill_h * c->fill_h);
         if (L.fill_list) {
             // all passes in one cooperative launch over the compacted list of masked voxels
             const float* a_cbct = cbct; float* a_A = L.A; float* a_B = L.B; unsigned char* a_xi = L.xi;
-            const unsigned* a_list = L.fill_list;
+            unsigned* a_list = L.fill_list; unsigned* a_list2 = L.fill_list + L.N; unsigned* a_q = L.fill_queued;
             int a_nx = L.nx, a_ny = L.ny, a_nz = L.nz, a_rt = c->fill_radius, a_max = c->max_fill_passes;
             float a_h = inv_h2; MaskCtl* a_ctl = c->d_mask; IterCtl a_ictl = ctl;
-            void* args[] = {&a_cbct, &a_A, &a_B, &a_xi, &a_list, &a_nx, &a_ny, &a_nz, &a_rt, &a_h, &a_max, &a_ctl, &a_ictl};
+            void* args[] = {&a_cbct, &a_A, &a_B, &a_xi, &a_list, &a_list2, &a_q, &a_nx, &a_ny, &a_nz, &a_rt, &a_h, &a_max, &a_ctl, &a_ictl};
             cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_fill_list, dim3(c->fill_grid), dim3(256), args, 0, st);
             if (e != cudaSuccess) return fail(c, DISC_ERR_CUDA, "k_fill_list: %s", cudaGetErrorString(e));
             DISC_TRY(check_launch(c, "k_fill_list"));
@@ -268,7 +278,7 @@ disc_status correct_ab(disc_ctx* c, const Level& L, const float* cbct, const flo
             }
         }
     } else {
-        k_ab_mask<false><<<g, 256, 0, st>>>(m, cbct, L.mu_s, L.var_s, L.A, L.B, nullptr, L.N, DISC_EPS_VAR, c->d_mask, ctl, nullptr);
+        k_ab_mask<false><<<g, 256, 0, st>>>(m, cbct, L.mu_s, L.var_s, L.A, L.B, nullptr, L.N, DISC_EPS_VAR, c->d_mask, ctl, nullptr, nullptr);
         DISC_TRY(check_launch(c, "k_ab"));
     }
     k_apply_ab<<<g, 256, 0, st>>>(cbct, L.A, L.B, out, L.N, c->d_partial, c->d_mask, slot >= 0 ? c->d_mean_a : nullptr,
@@ -485,6 +495,7 @@ disc_status disc_set_mask(disc_ctx* c, int enable, float hu0, float a_min, float
     DISC_NEED(c, h > 0.f, "h <= 0");
     DISC_NEED(c, max_fill_passes >= 1 && max_fill_passes <= 254, "max_fill_passes must be in 1..254");
     DISC_TRY(alloc_ab(c));
+    DISC_TRY(fill_grid_for(c, &c->fill_grid));
     c->mask_on = 1;
     c->mask_hu0 = hu0 >= 0.f ? hu0 : -1.f;
     c->mask_a_min = a_min >= 0.f ? a_min : -1.f;
